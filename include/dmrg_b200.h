@@ -1,0 +1,162 @@
+/*
+ * dmrg_b200.h — C ABI of the B200-native two-site DMRG effective-Hamiltonian library.
+ *
+ * The calls follow the problem statement of arxiv 2501.18263 (cited as PAPER.md:<line>):
+ *   - the quantum-chemistry Hamiltonian, Eq. (1), with the 1/2 in front of
+ *     the two-body sum (reading R1):
+ *       H = sum_{ij,s} T_ij a+_{is} a_{js} + 1/2 sum_{ijkl,s,t} V_ijkl a+_{is} a+_{jt} a_{lt} a_{ks} + e_core
+ *   - the MPS of PAPER.md Eq. (4) with U(1)xU(1) block-sparse tensors
+ *   - the two-site effective space H_L (x) H_k (x) H_{k+1} (x) H_R
+ *   - H_eff.psi as the task list of PAPER.md Eq. (6)-(8)
+ *   - the "iterative eigensolver" of PAPER.md:63 (Davidson, DESIGN.md App. E)
+ *   - the "renormalization steps" of PAPER.md:99 (operator blocking with an MPS tensor).
+ *
+ * Conventions:
+ *   orbitals i = 0..L-1 along the chain; sites are 1-based in the API (site i = orbital i-1);
+ *   site state s = 0..3 = {empty, down, up, up+down}, quantum numbers q(s) = (n_up, n_dn)
+ *   = (0,0),(0,1),(1,0),(1,1), |3> = a+_up a+_dn |0>;
+ *   bond b = 0..L lies between site b and b+1; a bond sector label q = (n_up, n_dn) counts the
+ *   electrons in sites 1..b.  All matrices are row-major doubles.
+ *
+ * Memory and errors:
+ *   Every function returns 0 on success and a negative dmrg_status on failure; the message of the
+ *   last failure on a context is dmrg_last_error(ctx).  No exception crosses the boundary and there
+ *   is no global state.  Pointers named h_* are HOST pointers (caller-owned, copied on entry or
+ *   filled on return); pointers named d_* are DEVICE pointers on the context's device.  Device
+ *   memory is obtained only through the allocator callbacks given at creation (the Python binding
+ *   backs them with torch tensors); `stream` arguments are a cudaStream_t passed as void* and all
+ *   device work of a call is enqueued on it.  Calls that return host results synchronise `stream`
+ *   before returning; dmrg_heff_apply and dmrg_heff_diag do not synchronise.
+ *   There is no CPU fallback: every numerical step runs in the library's CUDA kernels.
+ */
+#ifndef DMRG_B200_H
+#define DMRG_B200_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+  DMRG_OK = 0,
+  DMRG_ERR_ARG = -1,      /* invalid argument or call order */
+  DMRG_ERR_INPUT = -2,    /* input violates a stated requirement (symmetry, isometry, shapes) */
+  DMRG_ERR_ALLOC = -3,    /* allocator callback returned NULL */
+  DMRG_ERR_CUDA = -4,     /* CUDA runtime error (message holds cudaGetErrorString) */
+  DMRG_ERR_UNSUPPORTED = -5
+} dmrg_status;
+
+typedef struct dmrg_ctx dmrg_ctx;
+
+/* Device allocator callbacks.  alloc returns a device pointer aligned to >= 256 bytes or NULL. */
+typedef void* (*dmrg_alloc_fn)(uint64_t bytes, void* user);
+typedef void (*dmrg_free_fn)(void* ptr, void* user);
+
+typedef struct {
+  int32_t L;            /* number of spatial orbitals ("d") */
+  int32_t n_up, n_dn;   /* target electron numbers (N_alpha, N_beta); S_z = (n_up - n_dn)/2 */
+  int32_t symmetry;     /* 0 = U(1)xU(1).  1 = SU(2) is reserved: DMRG_ERR_UNSUPPORTED */
+  int32_t device;       /* CUDA device ordinal */
+  uint64_t workspace_bytes; /* cap for the intermediate (O_L.psi) buffer; 0 = library default */
+  dmrg_alloc_fn alloc;
+  dmrg_free_fn free;
+  void* alloc_user;
+} dmrg_config;
+
+int dmrg_create(const dmrg_config* cfg, dmrg_ctx** out);
+int dmrg_destroy(dmrg_ctx* ctx);
+const char* dmrg_last_error(const dmrg_ctx* ctx);
+
+/* PAPER.md Eq. (1).  h_T: L*L, h_V: L^4 with V[((i*L+j)*L+k)*L+l] the coefficient of
+ * 1/2 a+_{is} a+_{jt} a_{lt} a_{ks}.  Requires T symmetric and V_ijkl = V_klij to 1e-12 (else
+ * DMRG_ERR_INPUT).  The library uses w_ijkl = (V_ijkl + V_jilk)/2. */
+int dmrg_load_integrals(dmrg_ctx* ctx, int32_t L, const double* h_T, const double* h_V, double e_core);
+
+/* Bond sectors of the MPS (Eq. (4), :107).  For bond b = 0..L, sectors
+ * sec_off[b] .. sec_off[b+1]-1 of the arrays (q_up, q_dn, dim), sorted lexicographically by
+ * (q_up, q_dn) inside a bond.  Bond 0 must be {(0,0):1}, bond L {(n_up,n_dn):1}. */
+int dmrg_mps_set_sectors(dmrg_ctx* ctx, const int32_t* h_sec_off /* L+2 */, const int32_t* h_q_up,
+                         const int32_t* h_q_dn, const int32_t* h_dim);
+
+/* Site tensor of site i (1-based).  Blocks are listed as (q_in index within bond i-1, site state s);
+ * block n is the d_in x d_out matrix at h_data + blk_off[n], q_out = q_in + q(s) must be a sector of
+ * bond i.  canonical = 0: left-canonical (sum_{q_in,s} A^T A = 1 on each q_out), 1: right-canonical
+ * (sum_{s,q_out} A A^T = 1 on each q_in); violated beyond 1e-10 -> DMRG_ERR_INPUT. */
+int dmrg_mps_set_site(dmrg_ctx* ctx, int32_t site, int32_t canonical, int32_t nblocks,
+                      const int32_t* h_qin_idx, const int32_t* h_s, const int64_t* h_blk_off,
+                      const double* h_data, void* stream);
+
+/* Build the left environment from sites 1..k-1 and the right one from sites k+2..L by exact operator
+ * blocking, then prepare the two-site problem at bond (k, k+1): complementary
+ * operators, the task list of PAPER.md Eq. (8), and the diagonal of H_eff. */
+int dmrg_env_build(dmrg_ctx* ctx, int32_t k, void* stream);
+
+/* One renormalisation step: absorb site k into the left block (direction = 0, the
+ * left-canonical tensor of site k must have been set) or site k+1 into the right block
+ * (direction = 1), and prepare the two-site problem at the shifted bond (k+1,k+2) or (k-1,k).
+ * The environment on the other side is rebuilt from the stored site tensors if needed. */
+int dmrg_renormalize(dmrg_ctx* ctx, int32_t direction, void* stream);
+
+/* Layout of the two-site wavefunction Psi_{a, s_k, s_{k+1}, b}: blocks ordered by
+ * (q_L lexicographic, s_k, s_{k+1}); block n is a d_L x d_R row-major matrix at offset off[n] of the
+ * flat vector.  Pass NULL arrays to query only *nblocks / *n. */
+typedef struct {
+  int32_t qL_up, qL_dn;   /* label of bond k-1 */
+  int32_t s1, s2;         /* site states of sites k, k+1 */
+  int32_t qR_up, qR_dn;   /* label of bond k+1 (electrons in sites 1..k+1) */
+  int32_t dL, dR;
+  int64_t off;
+} dmrg_psi_block;
+int dmrg_psi_layout(dmrg_ctx* ctx, int32_t* nblocks, dmrg_psi_block* h_blocks, int64_t* n);
+
+/* psi_out = H_eff psi_in (Eq. (7)/(8)); e_core is included.  Overwrites d_psi_out. */
+int dmrg_heff_apply(dmrg_ctx* ctx, const double* d_psi_in, double* d_psi_out, void* stream);
+
+/* Diagonal of H_eff in the psi layout. */
+int dmrg_heff_diag(dmrg_ctx* ctx, double* d_diag, void* stream);
+
+/* Davidson for the lowest eigenpair (DESIGN.md App. E).  d_psi holds the start vector on entry and
+ * the normalised Ritz vector on return.  *iters = number of H_eff applications. */
+int dmrg_davidson(dmrg_ctx* ctx, double* d_psi, double tol, int32_t max_iter, int32_t max_basis,
+                  double* h_energy, int32_t* h_iters, double* h_resid, void* stream);
+
+/* Convenience end-to-end variants with HOST vectors (copies inside the call). */
+int dmrg_heff_apply_host(dmrg_ctx* ctx, const double* h_psi_in, double* h_psi_out, void* stream);
+int dmrg_davidson_host(dmrg_ctx* ctx, double* h_psi, double tol, int32_t max_iter, int32_t max_basis,
+                       double* h_energy, int32_t* h_iters, double* h_resid, void* stream);
+
+typedef struct {
+  int64_t n_terms;          /* four-part terms of PAPER.md Eq. (6) after pre-summation */
+  int64_t n_tasks;          /* (term x sector) tasks of PAPER.md Eq. (8) */
+  int64_t n_groups;         /* batched task groups handed to the kernel */
+  double flops_apply;       /* analytic: sum over tasks of the cheaper contraction order */
+  double flops_executed;    /* flops the kernels issue for one apply (padding included) */
+  double bytes_unique;      /* operator blocks once + psi in/out */
+  double bytes_intermediate;/* O_L.psi intermediates written+read per apply */
+  int64_t psi_size;         /* length of the flat psi vector */
+  int64_t op_bytes_left, op_bytes_right;
+  int32_t n_chunks;         /* workspace chunks per apply */
+  int32_t launches_per_apply;
+  double last_build_ms;     /* host+device time of the last dmrg_env_build / dmrg_renormalize */
+  double flops_renorm;      /* analytic flops of the last renormalisation step */
+  int64_t total_launches;   /* kernels launched by this context so far */
+} dmrg_stats_t;
+int dmrg_stats(dmrg_ctx* ctx, dmrg_stats_t* out);
+
+/* Export one carried block operator (for parity tests).  side 0 = left, 1 = right.  kind:
+ * 0 H, 1 C_up, 2 C_dn, 3 A_upup, 4 A_updn, 5 A_dndn, 6 B_upup, 7 B_updn, 8 B_dndn, 9 S_up, 10 S_dn.
+ * (i, j) are orbital indices (j ignored for one-index kinds).  The operator is returned as a dense
+ * (D x D) row-major matrix over the block's states in sector order, D = sum of sector dims.
+ * Right-block sectors are ordered by their bond label (electrons LEFT of the bond). */
+int dmrg_env_export(dmrg_ctx* ctx, int32_t side, int32_t kind, int32_t i, int32_t j,
+                    double* h_out, int64_t* D);
+
+/* Measured FP64 tensor-pipe (DMMA) peak of the device in TFLOP/s: a register-only mma loop on all
+ * SMs, timed with CUDA events on `stream`. */
+int dmrg_fp64_peak(dmrg_ctx* ctx, double* h_tflops, void* stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

@@ -1,0 +1,266 @@
+"""Thin ctypes binding of libdmrg_b200.so (include/dmrg_b200.h): argument marshalling only.
+
+Every numerical step runs in the library's CUDA kernels.  PyTorch is used for device memory (the
+allocator callbacks hand out torch uint8 tensors) and for the current CUDA stream.  There is no
+CPU fallback: importing works without a GPU (so that the symbol table can be checked), but
+`DMRG(...)` raises if CUDA or the shared library is missing.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+from . import build as _build
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libdmrg_b200.so")
+
+EXPORTS = [
+    "dmrg_create", "dmrg_destroy", "dmrg_last_error", "dmrg_load_integrals", "dmrg_mps_set_sectors",
+    "dmrg_mps_set_site", "dmrg_env_build", "dmrg_renormalize", "dmrg_psi_layout", "dmrg_heff_apply",
+    "dmrg_heff_diag", "dmrg_davidson", "dmrg_heff_apply_host", "dmrg_davidson_host", "dmrg_stats",
+    "dmrg_env_export", "dmrg_fp64_peak",
+]
+
+ALLOC_FN = C.CFUNCTYPE(C.c_void_p, C.c_uint64, C.c_void_p)
+FREE_FN = C.CFUNCTYPE(None, C.c_void_p, C.c_void_p)
+
+
+class Config(C.Structure):
+    _fields_ = [("L", C.c_int32), ("n_up", C.c_int32), ("n_dn", C.c_int32), ("symmetry", C.c_int32),
+                ("device", C.c_int32), ("workspace_bytes", C.c_uint64), ("alloc", ALLOC_FN),
+                ("free", FREE_FN), ("alloc_user", C.c_void_p)]
+
+
+class PsiBlock(C.Structure):
+    _fields_ = [("qL_up", C.c_int32), ("qL_dn", C.c_int32), ("s1", C.c_int32), ("s2", C.c_int32),
+                ("qR_up", C.c_int32), ("qR_dn", C.c_int32), ("dL", C.c_int32), ("dR", C.c_int32),
+                ("off", C.c_int64)]
+
+
+class Stats(C.Structure):
+    _fields_ = [("n_terms", C.c_int64), ("n_tasks", C.c_int64), ("n_groups", C.c_int64),
+                ("flops_apply", C.c_double), ("flops_executed", C.c_double), ("bytes_unique", C.c_double),
+                ("bytes_intermediate", C.c_double), ("psi_size", C.c_int64), ("op_bytes_left", C.c_int64),
+                ("op_bytes_right", C.c_int64), ("n_chunks", C.c_int32), ("launches_per_apply", C.c_int32),
+                ("last_build_ms", C.c_double), ("flops_renorm", C.c_double), ("total_launches", C.c_int64)]
+
+    def as_dict(self):
+        return {f: getattr(self, f) for f, _ in self._fields_}
+
+
+_lib = None
+
+
+def load_library(build_if_missing: bool = True):
+    """dlopen the in-tree shared library (building it with nvcc first if it is absent)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        if not build_if_missing:
+            raise RuntimeError("libdmrg_b200.so is missing: run `python -m paper_2501_18263_b200.build`")
+        _build.build()
+    lib = C.CDLL(LIB_PATH)
+    vp, i32, i64, dp = C.c_void_p, C.c_int32, C.c_int64, C.POINTER(C.c_double)
+    lib.dmrg_create.argtypes = [C.POINTER(Config), C.POINTER(vp)]
+    lib.dmrg_destroy.argtypes = [vp]
+    lib.dmrg_last_error.argtypes = [vp]
+    lib.dmrg_last_error.restype = C.c_char_p
+    lib.dmrg_load_integrals.argtypes = [vp, i32, vp, vp, C.c_double]
+    lib.dmrg_mps_set_sectors.argtypes = [vp, vp, vp, vp, vp]
+    lib.dmrg_mps_set_site.argtypes = [vp, i32, i32, i32, vp, vp, vp, vp, vp]
+    lib.dmrg_env_build.argtypes = [vp, i32, vp]
+    lib.dmrg_renormalize.argtypes = [vp, i32, vp]
+    lib.dmrg_psi_layout.argtypes = [vp, C.POINTER(i32), C.POINTER(PsiBlock), C.POINTER(i64)]
+    lib.dmrg_heff_apply.argtypes = [vp, vp, vp, vp]
+    lib.dmrg_heff_diag.argtypes = [vp, vp, vp]
+    lib.dmrg_davidson.argtypes = [vp, vp, C.c_double, i32, i32, dp, C.POINTER(i32), dp, vp]
+    lib.dmrg_heff_apply_host.argtypes = [vp, vp, vp, vp]
+    lib.dmrg_davidson_host.argtypes = [vp, vp, C.c_double, i32, i32, dp, C.POINTER(i32), dp, vp]
+    lib.dmrg_stats.argtypes = [vp, C.POINTER(Stats)]
+    lib.dmrg_env_export.argtypes = [vp, i32, i32, i32, i32, vp, C.POINTER(i64)]
+    lib.dmrg_fp64_peak.argtypes = [vp, dp, vp]
+    for name in EXPORTS:
+        if name != "dmrg_last_error":
+            getattr(lib, name).restype = C.c_int
+    _lib = lib
+    return lib
+
+
+class DMRGError(RuntimeError):
+    pass
+
+
+def _np_ptr(a):
+    return a.ctypes.data_as(C.c_void_p)
+
+
+class DMRG:
+    """One library context on one GPU.  Methods carry the names of the C calls (without `dmrg_`)."""
+
+    def __init__(self, L, n_up, n_dn, device=0, workspace_bytes=0):
+        import torch
+        if not torch.cuda.is_available():
+            raise DMRGError("CUDA device required: the library has no CPU path")
+        self.torch = torch
+        self.lib = load_library()
+        self.device = torch.device("cuda", device)
+        self._live = {}
+
+        def _alloc(nbytes, _user):
+            try:
+                t = torch.empty(int(nbytes), dtype=torch.uint8, device=self.device)
+            except Exception:  # out of memory -> NULL, the library reports DMRG_ERR_ALLOC
+                return None
+            self._live[t.data_ptr()] = t
+            return t.data_ptr()
+
+        def _free(ptr, _user):
+            self._live.pop(ptr, None)
+
+        self._alloc_cb = ALLOC_FN(_alloc)
+        self._free_cb = FREE_FN(_free)
+        self.cfg = Config(L, n_up, n_dn, 0, device, workspace_bytes, self._alloc_cb, self._free_cb, None)
+        self.ctx = C.c_void_p()
+        rc = self.lib.dmrg_create(C.byref(self.cfg), C.byref(self.ctx))
+        if rc != 0:
+            raise DMRGError("dmrg_create failed with status %d" % rc)
+        self.L, self.n_up, self.n_dn = L, n_up, n_dn
+
+    # -- plumbing --
+    def _check(self, rc):
+        if rc != 0:
+            raise DMRGError("status %d: %s" % (rc, self.lib.dmrg_last_error(self.ctx).decode()))
+
+    def _stream(self):
+        return C.c_void_p(self.torch.cuda.current_stream(self.device).cuda_stream)
+
+    def close(self):
+        if self.ctx:
+            self.lib.dmrg_destroy(self.ctx)
+            self.ctx = C.c_void_p()
+            self._live.clear()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # -- the C calls --
+    def load_integrals(self, T, V, e_core=0.0):
+        T = np.ascontiguousarray(T, dtype=np.float64)
+        V = np.ascontiguousarray(V, dtype=np.float64)
+        self._check(self.lib.dmrg_load_integrals(self.ctx, self.L, _np_ptr(T), _np_ptr(V), float(e_core)))
+
+    def mps_set_sectors(self, sectors):
+        """sectors: list over bonds 0..L of dict (n_up, n_dn) -> dim."""
+        off, qu, qd, dim = [0], [], [], []
+        self._sec_index = []
+        for sec in sectors:
+            keys = sorted(sec)
+            self._sec_index.append({q: i for i, q in enumerate(keys)})
+            for q in keys:
+                qu.append(q[0]); qd.append(q[1]); dim.append(sec[q])
+            off.append(len(qu))
+        a = [np.asarray(x, dtype=np.int32) for x in (off, qu, qd, dim)]
+        self._check(self.lib.dmrg_mps_set_sectors(self.ctx, *[_np_ptr(x) for x in a]))
+
+    def mps_set_site(self, site, canonical, blocks):
+        """blocks: dict (q_in, s) -> (d_in, d_out) array, site 1-based, canonical 0 left / 1 right."""
+        keys = sorted(blocks)
+        qin = np.asarray([self._sec_index[site - 1][k[0]] for k in keys], dtype=np.int32)
+        s = np.asarray([k[1] for k in keys], dtype=np.int32)
+        offs, parts, o = [], [], 0
+        for k in keys:
+            a = np.ascontiguousarray(blocks[k], dtype=np.float64)
+            offs.append(o); parts.append(a.reshape(-1)); o += a.size
+        data = np.concatenate(parts) if parts else np.zeros(1)
+        offs = np.asarray(offs, dtype=np.int64)
+        self._check(self.lib.dmrg_mps_set_site(self.ctx, site, canonical, len(keys), _np_ptr(qin), _np_ptr(s),
+                                               _np_ptr(offs), _np_ptr(data), self._stream()))
+
+    def env_build(self, k):
+        self._check(self.lib.dmrg_env_build(self.ctx, k, self._stream()))
+
+    def renormalize(self, direction):
+        self._check(self.lib.dmrg_renormalize(self.ctx, direction, self._stream()))
+
+    def psi_layout(self):
+        nb, n = C.c_int32(), C.c_int64()
+        self._check(self.lib.dmrg_psi_layout(self.ctx, C.byref(nb), None, C.byref(n)))
+        arr = (PsiBlock * nb.value)()
+        self._check(self.lib.dmrg_psi_layout(self.ctx, C.byref(nb), arr, C.byref(n)))
+        return list(arr), n.value
+
+    def psi_size(self):
+        nb, n = C.c_int32(), C.c_int64()
+        self._check(self.lib.dmrg_psi_layout(self.ctx, C.byref(nb), None, C.byref(n)))
+        return n.value
+
+    def heff_apply(self, psi_in, psi_out=None):
+        """psi_in: float64 CUDA tensor of length psi_size(); returns psi_out (CUDA tensor)."""
+        t = self.torch
+        assert psi_in.is_cuda and psi_in.dtype == t.float64 and psi_in.is_contiguous()
+        if psi_out is None:
+            psi_out = t.empty_like(psi_in)
+        self._check(self.lib.dmrg_heff_apply(self.ctx, C.c_void_p(psi_in.data_ptr()), C.c_void_p(psi_out.data_ptr()),
+                                             self._stream()))
+        return psi_out
+
+    def heff_diag(self):
+        t = self.torch
+        d = t.empty(self.psi_size(), dtype=t.float64, device=self.device)
+        self._check(self.lib.dmrg_heff_diag(self.ctx, C.c_void_p(d.data_ptr()), self._stream()))
+        return d
+
+    def davidson(self, psi, tol=1e-10, max_iter=200, max_basis=20):
+        """psi: CUDA start vector, overwritten with the Ritz vector.  Returns (energy, iters, resid)."""
+        e, it, r = C.c_double(), C.c_int32(), C.c_double()
+        self._check(self.lib.dmrg_davidson(self.ctx, C.c_void_p(psi.data_ptr()), tol, max_iter, max_basis,
+                                           C.byref(e), C.byref(it), C.byref(r), self._stream()))
+        return e.value, it.value, r.value
+
+    def heff_apply_host(self, psi_in: np.ndarray, psi_out: np.ndarray | None = None):
+        psi_in = np.ascontiguousarray(psi_in, dtype=np.float64)
+        if psi_out is None:
+            psi_out = np.empty_like(psi_in)
+        self._check(self.lib.dmrg_heff_apply_host(self.ctx, _np_ptr(psi_in), _np_ptr(psi_out), self._stream()))
+        return psi_out
+
+    def davidson_host(self, psi: np.ndarray, tol=1e-10, max_iter=200, max_basis=20):
+        assert psi.dtype == np.float64 and psi.flags.c_contiguous
+        e, it, r = C.c_double(), C.c_int32(), C.c_double()
+        self._check(self.lib.dmrg_davidson_host(self.ctx, _np_ptr(psi), tol, max_iter, max_basis,
+                                                C.byref(e), C.byref(it), C.byref(r), self._stream()))
+        return e.value, it.value, r.value
+
+    def stats(self):
+        s = Stats()
+        self._check(self.lib.dmrg_stats(self.ctx, C.byref(s)))
+        return s.as_dict()
+
+    def env_export(self, side, kind, i, j=0):
+        D = C.c_int64()
+        self._check(self.lib.dmrg_env_export(self.ctx, side, kind, i, j, None, C.byref(D)))
+        out = np.zeros((D.value, D.value))
+        self._check(self.lib.dmrg_env_export(self.ctx, side, kind, i, j, _np_ptr(out), C.byref(D)))
+        return out
+
+    def fp64_peak(self):
+        v = C.c_double()
+        self._check(self.lib.dmrg_fp64_peak(self.ctx, C.byref(v), self._stream()))
+        return v.value
+
+    # -- convenience: load everything a two-site problem needs from the generator objects --
+    def setup(self, T, V, mps, e_core=0.0):
+        self.load_integrals(T, V, e_core)
+        self.mps_set_sectors(mps.sectors)
+        for i, blocks in mps.left.items():
+            self.mps_set_site(i, 0, blocks)
+        for i, blocks in mps.right.items():
+            self.mps_set_site(i, 1, blocks)
+        self.env_build(mps.k)

@@ -1,0 +1,57 @@
+// Auxiliary kernels: psi pack/unpack between the compact C-ABI layout and the zero-padded internal
+// layout, the HBM-bound Davidson vector operations (DESIGN.md App. E), the H_eff diagonal, and the
+// DMMA peak probe.
+#pragma once
+#include <cuda_runtime.h>
+
+#include <cstdint>
+
+namespace dmrg {
+
+struct PsiBlockDev {
+  long long off_c;   // offset in the compact vector
+  long long off_p;   // offset in the padded vector
+  int rows, cols, rows_p, cols_p;
+};
+
+struct DiagTask {
+  const double* L;   // block of the left operator (or nullptr = identity)
+  const double* R;
+  long long rsL, rsR;
+  int ldl, ldr;
+  int count;
+  int pad_;
+  double alpha;
+};
+
+// padded[blocks] = compact (pads untouched: caller keeps them zero)
+void launch_pack(const PsiBlockDev* blocks, int nblocks, const double* compact, double* padded, cudaStream_t st);
+// compact = padded + shift * x_compact  (x_compact may be nullptr when shift == 0)
+void launch_unpack(const PsiBlockDev* blocks, int nblocks, const double* padded, double* compact,
+                   double shift, const double* x_compact, cudaStream_t st);
+
+constexpr int DOT_BLOCKS = 592;   // 4 per SM, fixed => deterministic reduction tree
+// out[j] = sum_i x[i] * Y[j*ldy + i], j < m   (two kernels; `partials` holds m*DOT_BLOCKS doubles)
+void launch_multidot(const double* x, const double* Y, long long ldy, int m, long long n,
+                     double* partials, double* out, cudaStream_t st);
+// y = sum_j c[j] * V[j*ldv + i]  (c on device, m <= 64)
+void launch_combine(const double* V, long long ldv, const double* c, int m, long long n, double* y, cudaStream_t st);
+// y += a * x
+void launch_axpy(double a, const double* x, double* y, long long n, cudaStream_t st);
+// y -= sum_j c[j] * V[j]   (c on device)
+void launch_project_out(const double* V, long long ldv, const double* c, int m, long long n, double* y, cudaStream_t st);
+// y += a (every element)
+void launch_add_const(double a, double* y, long long n, cudaStream_t st);
+// y = a * y
+void launch_scale(double a, double* y, long long n, cudaStream_t st);
+// t = r / clamp(theta - d)   with |theta - d| >= 1e-12, sign kept; r = hx - theta*x computed on the fly
+void launch_residual_precond(const double* x, const double* hx, const double* d, double theta,
+                             double* r, double* t, long long n, cudaStream_t st);
+// diag(H_eff): out_p[block] = sum_tasks alpha * diag(L) (x) diag(R)
+void launch_diag(const PsiBlockDev* blocks, int nblocks, const DiagTask* tasks, const int* task_begin,
+                 double* out_p, cudaStream_t st);
+// register-only DMMA loop; returns achieved TFLOP/s
+constexpr int DIAG_MAX_DIM = 640;
+cudaError_t measure_dmma_peak(double* d_scratch, double* tflops, cudaStream_t st);
+
+}  // namespace dmrg

@@ -1,0 +1,119 @@
+// Host-side model: sectors, block-sparse operator classes, MPS tensors, and the context.
+//
+// Operator storage ("class storage"): operators of one kind on one
+// block share q_out - q_in = (du, dd) and therefore their block structure.  A class
+// stores, for each non-zero block (q_out, q_in), ALL its operators contiguously:
+//     data[ block.off + op * rp * cp + r * cp + c ],   rp, cp = dims padded to multiples of 8
+// so that "one block of every operator in a term group" is a strided batch for the GEMM kernel.
+#pragma once
+#include <array>
+#include <map>
+#include <memory>
+
+#include "common.h"
+#include "kernels.cuh"
+#include "plan.h"
+
+namespace dmrg {
+
+static const int SITE_QU[4] = {0, 0, 1, 1};   // s = 0, dn, up, up+dn
+static const int SITE_QD[4] = {0, 1, 0, 1};
+
+struct Sectors {
+  std::vector<int> qu, qd, dim;
+  std::unordered_map<int, int> index;
+  static int key(int u, int d) { return (u + 256) * 4096 + (d + 256); }
+  int size() const { return (int)dim.size(); }
+  int find(int u, int d) const {
+    auto it = index.find(key(u, d));
+    return it == index.end() ? -1 : it->second;
+  }
+  void add(int u, int d, int n) {
+    index[key(u, d)] = size();
+    qu.push_back(u); qd.push_back(d); dim.push_back(n);
+  }
+  long long total() const { long long t = 0; for (int x : dim) t += x; return t; }
+};
+
+enum Kind : int { K_ID = 0, K_H, K_CU, K_CD, K_AUU, K_AUD, K_ADD, K_BUU, K_BUD, K_BDD, K_SU, K_SD, K_NSTD };
+
+struct ClsBlock {
+  int so, si;          // out / in sector index
+  int rows, cols, rp, cp;
+  long long off;       // element offset of operator 0 of this block
+};
+
+struct OpClass {
+  int kind = 0, du = 0, dd = 0, nops = 0, nalloc = 0;
+  std::vector<ClsBlock> blocks;
+  std::vector<int> blk_of_in, blk_of_out;
+  DevArray<double> data;
+  long long elems = 0;
+  void layout(const Sectors& sec, int du_, int dd_, int nops_);
+  void allocate(Allocator* al, cudaStream_t st);
+  double* ptr(int b, int r) const { return data.p + blocks[b].off + (long long)r * blocks[b].rp * blocks[b].cp; }
+  long long op_stride(int b) const { return (long long)blocks[b].rp * blocks[b].cp; }
+};
+
+struct BlockSide {
+  bool is_left = true;
+  int lo = 0, hi = 0;          // orbitals [lo, hi)
+  Sectors sec;                 // labelled by the block's own electron content
+  std::vector<std::unique_ptr<OpClass>> cls;   // [0, K_NSTD) standard kinds, then pre-summed classes
+  int norb() const { return hi - lo; }
+  uint64_t bytes() const { uint64_t b = 0; for (auto& c : cls) if (c) b += (uint64_t)c->elems * 8; return b; }
+};
+
+struct SiteBlk {
+  int qin, s, qout;            // sector indices in bond i-1 / bond i
+  int din, dout, dinp, doutp;
+  long long off;               // element offset in the padded device array
+};
+
+struct SiteTensor {
+  int canonical = -1;          // 0 left, 1 right, -1 unset
+  std::vector<SiteBlk> blks;
+  std::map<std::pair<int, int>, int> find;   // (qin, s) -> block
+  DevArray<double> data;
+};
+
+struct OpRef { int cls = K_ID; int idx = 0; bool tr = false; };
+
+struct SiteOpTable {
+  std::vector<std::array<double, 16>> mats;
+  SiteOpTable();
+  int intern(const double* m);
+  int parity(int id) const;
+};
+
+struct PsiBlk { int qL, s1, s2, qR; int dL, dR, dLp, dRp; long long off_c, off_p; };
+
+}  // namespace dmrg
+
+// The opaque context of the C ABI.
+struct dmrg_ctx {
+  dmrg_config cfg;
+  dmrg::Allocator al;
+  std::string err;
+  int L = 0;
+  std::vector<double> T, w;    // T (L*L), w_ijkl = (V_ijkl + V_jilk)/2 (L^4)
+  double e_core = 0;
+  bool have_integrals = false;
+  std::vector<dmrg::Sectors> bond;          // bond sectors, label = electrons left of the bond
+  std::vector<dmrg::SiteTensor> site;       // 1-based
+  int k = 0;                                // current bond (k, k+1); 0 = none
+  std::unique_ptr<dmrg::BlockSide> left, right;
+  dmrg::SiteOpTable site_ops;
+  // two-site problem
+  std::vector<dmrg::PsiBlk> psi;
+  std::map<std::array<int, 3>, int> psi_find;   // (qL, s1, s2) -> block
+  long long psi_n = 0, psi_np = 0;
+  dmrg::DevArray<dmrg::PsiBlockDev> d_psi_blocks;
+  dmrg::DevArray<double> psi_in_p, psi_out_p, diag_p;
+  dmrg::Plan apply_plan;
+  dmrg_stats_t stats{};
+  int64_t launches = 0;
+  // Davidson workspace
+  dmrg::DevArray<double> dav_V, dav_W, dav_tmp, dav_small, dav_partials;
+  int dav_basis = 0;
+};

@@ -1,0 +1,87 @@
+// Contraction planner: turns "C += alpha * X*Y*W" items (Eq. (8) tasks and the
+// renormalisation triple products of PAPER.md:99) into launches of the grouped GEMM kernel.
+//
+// A three-matrix item is executed in two phases inside one workspace chunk:
+//   phase 1:  Z[b] = X[b]*Y[b]   (or Y[b]*W[b], whichever order is cheaper)   -> workspace
+//   phase 2:  C   += alpha * Z[b]*W[b]   (or X[b]*Z[b])
+// Items that accumulate into the same output become K-segments of ONE output tile, so the sum over
+// terms stays in registers (no global atomics).  Chunks bound the workspace; outputs accumulate
+// across chunks (they are zeroed by the caller before the plan runs).
+#pragma once
+#include <map>
+#include <tuple>
+
+#include "common.h"
+#include "gemm.cuh"
+
+namespace dmrg {
+
+// A matrix operand.  Logical shape is (rows x cols) AFTER the optional transpose; `p` points to the
+// stored row-major array with leading dimension ld; element b of a batch is at p + b*stride.
+struct Mat {
+  const double* p = nullptr;
+  int ld = 0;
+  bool tr = false;          // stored array is the transpose of the logical matrix
+  long long stride = 0;
+  int rows = 0, cols = 0;   // padded logical dims (multiples of 8)
+  int urows = 0, ucols = 0; // unpadded logical dims (for the analytic flop count)
+};
+
+struct Item {
+  double* C = nullptr;
+  int ldc = 0;
+  long long strideC = 0;    // 0: all `count` products accumulate into the same C; else batch of outputs
+  int count = 1;
+  double alpha = 1.0;
+  int nmat = 2;             // C += alpha X*Y (2) or alpha X*Y*W (3)
+  Mat X, Y, W;
+};
+
+struct Phase {
+  DevArray<GOut> outs;
+  DevArray<GSeg> segs;
+  DevArray<GTile> tiles;
+  int ntiles = 0;
+};
+
+struct Chunk {
+  Phase p1, p2;
+};
+
+struct Plan {
+  std::vector<Chunk> chunks;
+  DevArray<double> workspace;
+  double flops_analytic = 0, flops_executed = 0, bytes_intermediate = 0;
+  int64_t n_items = 0, n_products = 0;
+  int launches() const;
+  void run(cudaStream_t st, int64_t* launch_counter) const;
+  void clear() { chunks.clear(); workspace.release(); }
+};
+
+class Planner {
+ public:
+  Planner(Allocator* al, uint64_t workspace_cap_bytes) : al_(al), cap_(workspace_cap_bytes / 8) {}
+  void add(const Item& it);
+  // Uploads descriptors, allocates the workspace and patches workspace-relative pointers.
+  void finish(Plan* plan, cudaStream_t st);
+
+ private:
+  struct HSeg { GSeg s; bool a_ws, b_ws; };          // *_ws: pointer is a workspace offset
+  struct HOut { GOut o; bool c_ws; std::vector<HSeg> segs; int batch; double work; };
+  struct HChunk {
+    std::vector<HOut> p1;
+    std::vector<HOut> p2;
+    std::map<std::tuple<const double*, int, long long>, int> p2_index;  // (C, batch, strideC) -> p2 slot
+    long long ws_used = 0;
+  };
+  void add_piece(const Item& it, int b0, int cnt);
+  HOut& p2_out(HChunk& ch, const Item& it, int b0, int cnt, int M, int N);
+  Allocator* al_;
+  long long cap_;
+  std::vector<HChunk> chunks_;
+  long long ws_max_ = 0;
+  double fa_ = 0, fe_ = 0, bi_ = 0;
+  int64_t n_items_ = 0, n_products_ = 0;
+};
+
+}  // namespace dmrg
