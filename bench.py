@@ -1,0 +1,294 @@
+#!/usr/bin/env python
+"""bench.py — H_eff.psi FP64 throughput at the middle bond (BASELINE.json `metric`).
+
+  python bench.py --gpus N --steps K --warmup W [--config C] [--impl reference]
+
+One "step" is one H_eff.psi (Eq. (7)/(8)) on the two-site problem of BASELINE.json
+configs[C] (default C = 3, the U(1)xU(1) D = 4096 problem the north_star target is quoted on; it fits
+one GPU).  The line also carries ms per Davidson iteration and one renormalisation step (the other
+rows of SURVEY.md 8(a)), the roofline object, the end-to-end number through the host-buffer C call,
+and the CPU oracle timed on a bounded sample.  N > 1: replicas only (the path does not shard,
+DESIGN.md "Multi-GPU"): every rank runs the same problem on its own GPU, no data-path collective.
+
+`--impl reference` times the CPU oracle (oracle/, as it stands) on the host cores.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "heff_apply_fp64_gflops"
+UNIT = "GFLOP/s"
+SAMPLE_CFG = 1   # bounded CPU sample: BASELINE.json configs[1] (L=20, D=256)
+
+
+class ClockSampler:
+    """Samples nvidia-smi clocks and throttle reasons during the timed region."""
+
+    def __init__(self, index):
+        self.index = index
+        self.rows = []
+        self.proc = None
+
+    def start(self):
+        q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+             "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + q,
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append(line.strip())
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": []}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            f = [x.strip() for x in r.split(",")]
+            if len(f) < 6:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1]))
+            except ValueError:
+                continue
+            for n, v in zip(names, f[2:6]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def time_oracle_sample(steps, warmup):
+    """The CPU oracle on BASELINE.json configs[1]; GFLOP/s from the flops its own matmuls execute."""
+    from oracle import dmrg as odmrg
+    from paper_2501_18263_b200 import inputs
+    T, V, mps = inputs.make_config(SAMPLE_CFG)
+    pb = inputs.psi_blocks(mps)
+    orc = odmrg.TwoSiteOracle(T, V, mps.n_up, mps.n_dn, mps.k, mps.sectors, mps.left, mps.right, pb)
+    orc.build_env()
+    orc.terms()
+    v = inputs.make_psi0(mps, inputs.CONFIGS[SAMPLE_CFG]["seed"])
+    flops = oracle_apply_flops(orc)
+    for _ in range(warmup):
+        orc.apply(v)
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        orc.apply(v)
+    dt = (time.perf_counter() - t0) / max(steps, 1)
+    try:
+        import threadpoolctl
+        cores = max(p["num_threads"] for p in threadpoolctl.threadpool_info()) if threadpoolctl.threadpool_info() else os.cpu_count()
+    except Exception:
+        cores = os.cpu_count()
+    return {"value": flops / dt * 1e-9, "unit": UNIT, "cores": int(cores), "kind": "oracle",
+            "sample": "BASELINE configs[%d] (L=20, N=(10,10), D=256, middle bond): %d H_eff.psi, %.2f s each; "
+                      "flops = those of the oracle's own block matmuls" % (SAMPLE_CFG, steps, dt),
+            "ms_per_apply": dt * 1e3}
+
+
+def oracle_apply_flops(orc):
+    """Flops of the matmuls one oracle apply executes (instrumentation only: shapes, no arithmetic)."""
+    psi_keys = {}
+    for (qL, s1, s2, qRb, dL, dR) in orc.psi_blocks:
+        from oracle.dmrg import SITE_Q, qsub
+        psi_keys[((qL, SITE_Q[s1]), (SITE_Q[s2], qsub(orc.N, qRb)))] = (dL, dR)
+    by_left = {}
+    for (kl, kr), shp in psi_keys.items():
+        by_left.setdefault(kl, []).append((kr, shp))
+    fl = 0.0
+    for XL, XR, hc in orc.terms():
+        r_in, r_out = {}, {}
+        for (kro, kri), mR in XR.items():
+            r_in.setdefault(kri, []).append((kro, mR.shape))
+            r_out.setdefault(kro, []).append((kri, mR.shape))
+        for (klo, kli), mL in XL.items():
+            for kri, (dl, dr) in by_left.get(kli, ()):
+                for kro, shp in r_in.get(kri, ()):
+                    if (klo, kro) in psi_keys:
+                        fl += 2.0 * mL.shape[0] * mL.shape[1] * dr + 2.0 * mL.shape[0] * dr * shp[0]
+            if hc:
+                for kro, (dl, dr) in by_left.get(klo, ()):
+                    for kri, shp in r_out.get(kro, ()):
+                        if (kli, kri) in psi_keys:
+                            fl += 2.0 * mL.shape[1] * mL.shape[0] * dr + 2.0 * mL.shape[1] * dr * shp[1]
+    return fl
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    cb = time_oracle_sample(max(args.steps, 1), min(args.warmup, 1))
+    line = {"impl": "reference", "metric": METRIC, "value": cb["value"], "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": cb["ms_per_apply"], "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": "cpu oracle on a bounded sample: " + cb["sample"]},
+            "cpu_baseline": cb,
+            "e2e": {"value": cb["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line))
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2501_18263_b200 import inputs
+    from paper_2501_18263_b200.binding import DMRG
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (no CPU fallback)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    cfg = args.config
+    c = inputs.CONFIGS[cfg]
+    D = args.D if args.D else (c["D"] if cfg != 4 else c["D"])
+    t0 = time.perf_counter()
+    T, V, mps = inputs.make_config(cfg, D=D)
+    d = DMRG(mps.L, mps.n_up, mps.n_dn, device=local, workspace_bytes=args.workspace_gb << 30)
+    d.setup(T, V, mps)
+    torch.cuda.synchronize()
+    setup_s = time.perf_counter() - t0
+    st = d.stats()
+    n = d.psi_size()
+    dev = torch.device("cuda", local)
+    x = torch.from_numpy(inputs.make_psi0(mps, c["seed"])).to(dev)
+    y = torch.empty_like(x)
+    peak_tf = d.fp64_peak()
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- device-resident: K applies.  The operator working set (tens of GB at config 3) is far larger
+    # than the 126 MB L2, so consecutive steps cannot reuse cached operands.
+    for _ in range(args.warmup):
+        d.heff_apply(x, y)
+    barrier()
+    sampler = ClockSampler(local)
+    sampler.start()
+    l0 = d.stats()["total_launches"]
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(args.steps):
+        d.heff_apply(x, y)
+    e1.record()
+    barrier()
+    clocks = sampler.stop()
+    launches = d.stats()["total_launches"] - l0
+    ms = e0.elapsed_time(e1) / args.steps
+    tmax = torch.tensor([ms], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
+    ms_max = float(tmax.item())
+    value = world * st["flops_apply"] / (ms_max * 1e-3) * 1e-9
+
+    # ---- end to end through the host-buffer C call (pinned host psi in, psi out)
+    hx = torch.from_numpy(inputs.make_psi0(mps, c["seed"])).pin_memory()
+    hy = torch.empty_like(hx).pin_memory()
+    hxn, hyn = hx.numpy(), hy.numpy()
+    d.heff_apply_host(hxn, hyn)
+    barrier()
+    t1 = time.perf_counter()
+    esteps = max(1, min(args.steps, 5))
+    for _ in range(esteps):
+        d.heff_apply_host(hxn, hyn)
+    torch.cuda.synchronize()
+    e2e_ms = (time.perf_counter() - t1) / esteps * 1e3
+    te = torch.tensor([e2e_ms], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(te, op=dist.ReduceOp.MAX)
+    e2e_val = world * st["flops_apply"] / (float(te.item()) * 1e-3) * 1e-9
+
+    extra = {}
+    if rank == 0 and not args.quick:
+        # ---- Davidson: fixed 10 iterations from the random start vector
+        dg = d.heff_diag()      # start: lowest diagonal element + 1 % random (R20)
+        z = 0.01 * x
+        z[int(torch.argmin(dg))] += 1.0
+        z /= torch.linalg.norm(z)
+        torch.cuda.synchronize()
+        t2 = time.perf_counter()
+        E, it, rn = d.davidson(z, tol=1e-30, max_iter=10, max_basis=12)
+        torch.cuda.synchronize()
+        extra["davidson"] = {"iters": it, "ms_per_iter": (time.perf_counter() - t2) * 1e3 / it, "energy": E, "resid": rn}
+        extra["env_build"] = {"setup_s": setup_s, "last_build_ms": st["last_build_ms"],
+                              "last_renorm_step_gflop": st["flops_renorm"] * 1e-9}
+
+    if rank == 0:
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+                "warmup": args.warmup, "ms_per_step": ms_max, "higher_is_better": True, "scaling": "weak",
+                "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+                "config": {"workload": "BASELINE configs[%d]: L=%d, N=(%d,%d), U(1)xU(1), D=%d, middle bond (%d,%d), "
+                                       "one H_eff.psi per step" % (cfg, mps.L, mps.n_up, mps.n_dn, D, mps.k, mps.k + 1),
+                           "psi_size": n, "terms": st["n_terms"], "tasks": st["n_tasks"],
+                           "flops_per_apply": st["flops_apply"], "operator_bytes": st["op_bytes_left"] + st["op_bytes_right"],
+                           "l2": "operator working set >> L2 (no flush needed)", "parallelism": "replicas" if world > 1 else "single"},
+                "clocks": clocks,
+                "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": 8 * n, "d2h_bytes_per_step": 8 * n,
+                        "ms_per_step": float(te.item())},
+                "gpu_launches": int(launches),
+                "roofline": {"bound": "tensor", "achieved": value / world * 1e-3, "peak": peak_tf, "unit": "TFLOP/s",
+                             "frac": value / world * 1e-3 / peak_tf, "traffic": None,
+                             "peak_source": "FP64 DMMA register-only loop measured in this run (dmrg_fp64_peak); "
+                                            "MEASURED_PEAKS.json has no FP64 entry",
+                             "kernel": "k_grouped_gemm (%d launches per H_eff.psi, timed as one apply)" % (st["launches_per_apply"] - 2),
+                             "flops_executed_per_apply": st["flops_executed"],
+                             "bytes_intermediate_per_apply": st["bytes_intermediate"]},
+                }
+        line.update(extra)
+        if world == 1 and not args.no_cpu:
+            line["cpu_baseline"] = time_oracle_sample(2, 1)
+        print(json.dumps(line))
+    d.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=3)
+    ap.add_argument("--D", type=int, default=0)
+    ap.add_argument("--workspace-gb", type=int, default=16, dest="workspace_gb")
+    ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--quick", action="store_true", help="skip the Davidson / renormalisation extras")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()
