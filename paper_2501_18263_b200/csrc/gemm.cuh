@@ -1,12 +1,13 @@
 // Grouped, batched, segment-accumulating FP64 GEMM on the DMMA pipe (sm_100a).
 //
-// One launch executes a list of output tiles.  Each output matrix C (M x N) is
+// One launch executes a list of output tiles of ONE tile shape.  Each output matrix C (M x N) is
 //     C (+)= sum_{seg in segs(C)} sum_{r < seg.count} alpha_seg * op(A_seg[r]) * op(B_seg[r])
 // which is the shape of every dense contraction on the DMRG hot path (Eq. (8), :109):
-//   phase 1 of a task group : Z_r   = O_L,r * Psi_in            (batch over r, one segment)
-//   phase 2 of an output    : Psi' += sum_r alpha Z_r * O_R,r^T  (segments accumulate in registers,
-//                                                                no global atomics)
-//   renormalisation         : O'   += A2^T (O A1)               (PAPER.md:99)
+//   phase 1 of a task group : Z     = [O_L,0; O_L,1; ..] * Psi_in   (operators of a term group stacked
+//                                                                    along M: "segmented rows")
+//   phase 2 of an output    : Psi' += sum_r alpha Z_r * O_R,r^T      (segments accumulate in registers,
+//                                                                    no global atomics)
+//   renormalisation         : O'   += A2^T (O A1)                    (PAPER.md:99)
 //   complementary operators : P     = W * [stacked normal operator blocks]
 // All dimensions are multiples of 8 (blocks are stored zero-padded), so no edge predication
 // inside an 8x8x4 mma tile is needed.
@@ -21,6 +22,11 @@ struct GSeg {
   const double* B;
   long long rsA, rsB;   // per-repeat strides in elements (repeats accumulate into one output)
   long long bsA, bsB;   // per-batch strides in elements (batch elements are separate outputs)
+  // segmented rows / columns: row m of op(A) lives in operator (m / amr) at A + (m / amr) * ams, local
+  // row m % amr (amr == 0: plain matrix).  Same for the columns of op(B) with bnr / bns.
+  long long ams, bns;
+  int amr, bnr;
+  unsigned amr_inv, bnr_inv;   // floor(2^32 / d) + 1 for the division by amr / bnr
   int lda, ldb;
   int K;                // multiple of 8
   int count;            // repeats accumulated into the same output
@@ -34,20 +40,21 @@ struct GOut {
   long long bsC;            // batch stride of C in elements
   int M, N, ldc;
   int seg_begin, seg_end;
-  int tile_m, tile_n;       // tile extents, multiples of 8, <= 128
   int accumulate;           // 1: C += acc, 0: C = acc
 };
 
 struct GTile {
-  int out, batch, tm, tn;   // output index, batch index, tile row / column index
+  int out, batch, m0, n0;   // output index, batch index, first row / column of the tile
 };
 
-constexpr int GEMM_BM = 128, GEMM_BN = 128, GEMM_KC = 16, GEMM_STAGES = 4, GEMM_THREADS = 256;
-constexpr int GEMM_STAGE_DOUBLES = 2 * GEMM_BM * (GEMM_KC + 4);
-constexpr int GEMM_SMEM_BYTES = GEMM_STAGES * GEMM_STAGE_DOUBLES * 8;
+// Tile shapes (rows x cols of C per CTA).  Index = 3 * row_class + col_class, classes {32, 64, 128}.
+constexpr int GEMM_NSHAPES = 9;
+constexpr int GEMM_DIMS[3] = {32, 64, 128};
+inline int gemm_shape_rows(int s) { return GEMM_DIMS[s / 3]; }
+inline int gemm_shape_cols(int s) { return GEMM_DIMS[s % 3]; }
 
-// Launch over `ntiles` tiles (device arrays).  Returns the cudaError of the launch.
-cudaError_t launch_grouped_gemm(const GOut* d_outs, const GSeg* d_segs, const GTile* d_tiles,
+// Launch `ntiles` tiles of shape `shape` (device arrays).  Returns the cudaError of the launch.
+cudaError_t launch_grouped_gemm(int shape, const GOut* d_outs, const GSeg* d_segs, const GTile* d_tiles,
                                 int ntiles, cudaStream_t stream);
 cudaError_t grouped_gemm_init();
 

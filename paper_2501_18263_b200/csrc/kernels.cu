@@ -145,6 +145,20 @@ __global__ void k_diag(const PsiBlockDev* __restrict__ blocks, const DiagTask* _
   }
 }
 
+__global__ void k_reduce_partials(const RedDesc* __restrict__ ds) {
+  const RedDesc d = ds[blockIdx.x];
+  const int b = blockIdx.y;
+  if (b >= d.batch) return;
+  const long long mn = (long long)d.M * d.N;
+  double* C = d.C + (long long)b * d.bsC;
+  for (long long e = threadIdx.x; e < mn; e += blockDim.x) {
+    const int r = (int)(e / d.N), c = (int)(e % d.N);
+    double s = C[(long long)r * d.ldc + c];
+    for (int p = 0; p < d.nparts; ++p) s += d.P[((long long)p * d.batch + b) * mn + e];
+    C[(long long)r * d.ldc + c] = s;
+  }
+}
+
 __global__ void k_dmma_peak(double* out, int iters, double a, double b) {
   double c[8][2];
 #pragma unroll
@@ -203,6 +217,10 @@ void launch_residual_precond(const double* x, const double* hx, const double* d,
 void launch_diag(const PsiBlockDev* blocks, int nblocks, const DiagTask* tasks, const int* task_begin,
                  double* out_p, cudaStream_t st) {
   if (nblocks > 0) k_diag<<<nblocks, 256, 0, st>>>(blocks, tasks, task_begin, out_p);
+}
+
+void launch_reduce_partials(const RedDesc* d, int n, int max_batch, cudaStream_t st) {
+  if (n > 0) k_reduce_partials<<<dim3(n, max_batch), 256, 0, st>>>(d);
 }
 
 cudaError_t measure_dmma_peak(double* dummy, double* tflops, cudaStream_t st) {

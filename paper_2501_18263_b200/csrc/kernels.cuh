@@ -50,6 +50,14 @@ void launch_residual_precond(const double* x, const double* hx, const double* d,
 // diag(H_eff): out_p[block] = sum_tasks alpha * diag(L) (x) diag(R)
 void launch_diag(const PsiBlockDev* blocks, int nblocks, const DiagTask* tasks, const int* task_begin,
                  double* out_p, cudaStream_t st);
+// split-K partial sums: C[b] += P[0][b] + P[1][b] + ... (fixed order => deterministic)
+struct RedDesc {
+  double* C;
+  const double* P;           // part p, batch b at P + (p * batch + b) * M * N, row-major with ld = N
+  long long bsC;
+  int M, N, ldc, nparts, batch, pad_;
+};
+void launch_reduce_partials(const RedDesc* d, int n, int max_batch, cudaStream_t st);
 // register-only DMMA loop; returns achieved TFLOP/s
 constexpr int DIAG_MAX_DIM = 640;
 cudaError_t measure_dmma_peak(double* d_scratch, double* tflops, cudaStream_t st);

@@ -7,24 +7,41 @@ namespace dmrg {
 
 int Plan::launches() const {
   int n = 0;
-  for (const auto& c : chunks) n += (c.p1.ntiles > 0) + (c.p2.ntiles > 0);
+  for (const auto& c : chunks) n += c.p1.launches() + c.p2.launches();
   return n;
+}
+
+static void run_phase(const Phase& ph, cudaStream_t st, int64_t* launch_counter) {
+  for (int s = GEMM_NSHAPES - 1; s >= 0; --s) {   // largest tiles first
+    if (ph.ntiles[s] <= 0) continue;
+    DMRG_CUDA(launch_grouped_gemm(s, ph.outs.p, ph.segs.p, ph.tiles[s].p, ph.ntiles[s], st));
+    if (launch_counter) ++*launch_counter;
+  }
+  if (ph.nred > 0) {
+    launch_reduce_partials(ph.red.p, ph.nred, ph.red_max_batch, st);
+    if (launch_counter) ++*launch_counter;
+  }
 }
 
 void Plan::run(cudaStream_t st, int64_t* launch_counter) const {
   for (const auto& c : chunks) {
-    if (c.p1.ntiles > 0) {
-      DMRG_CUDA(launch_grouped_gemm(c.p1.outs.p, c.p1.segs.p, c.p1.tiles.p, c.p1.ntiles, st));
-      if (launch_counter) ++*launch_counter;
-    }
-    if (c.p2.ntiles > 0) {
-      DMRG_CUDA(launch_grouped_gemm(c.p2.outs.p, c.p2.segs.p, c.p2.tiles.p, c.p2.ntiles, st));
-      if (launch_counter) ++*launch_counter;
-    }
+    run_phase(c.p1, st, launch_counter);
+    run_phase(c.p2, st, launch_counter);
   }
 }
 
 static inline double fl(double a, double b, double c) { return 2.0 * a * b * c; }
+
+// Splits an extent (multiple of 8) into tile rows/cols of class 0/1/2 = 32/64/128: (start, class).
+static void split_dim(int n, std::vector<std::pair<int, int>>& out) {
+  int pos = 0;
+  while (pos < n) {
+    int rem = n - pos;
+    if (rem > 96) { out.push_back({pos, 2}); pos += 128; }
+    else if (rem > 32) { out.push_back({pos, 1}); pos += 64; }
+    else { out.push_back({pos, 0}); pos += 32; }
+  }
+}
 
 void Planner::add(const Item& it) {
   DMRG_REQUIRE(it.count >= 1, DMRG_ERR_ARG, "planner: empty item");
@@ -71,6 +88,7 @@ void Planner::add_piece(const Item& it, int b0, int cnt) {
     h.s.A = A; h.s.B = B; h.s.lda = lda; h.s.ldb = ldb; h.s.K = K; h.s.count = 1;
     h.s.flags = (ta ? 1 : 0) | (tb ? 2 : 0); h.s.alpha = 1.0;
     h.s.rsA = h.s.rsB = h.s.bsA = h.s.bsB = 0; h.a_ws = h.b_ws = false;
+    h.s.ams = h.s.bns = 0; h.s.amr = h.s.bnr = 0; h.s.amr_inv = h.s.bnr_inv = 0;
     return h;
   };
   if (it.nmat == 2) {
@@ -97,16 +115,29 @@ void Planner::add_piece(const Item& it, int b0, int cnt) {
   ws_max_ = std::max(ws_max_, ch.ws_used);
   bi_ += 2.0 * 8.0 * zsz * cnt;
   fe_ += cnt * std::min(pl, pr);
-  // phase 1: Z[b] = X[b] Y[b]  or  Y[b] W[b]
+  // phase 1: Z[b] = X[b] Y[b]  or  Y[b] W[b].  When only one operand varies with b the `cnt` products
+  // are ONE GEMM: operators stacked along M (segmented rows of op(A)) or along N (segmented columns of
+  // op(B)); the class storage keeps them contiguous per block, so no copy is needed.
+  const Mat& A1 = left_first ? it.X : it.Y;
+  const Mat& B1 = left_first ? it.Y : it.W;
+  const bool mergeM = cnt > 1 && A1.stride != 0 && B1.stride == 0;
+  const bool mergeN = cnt > 1 && A1.stride == 0 && B1.stride != 0;
+  const long long zld = mergeN ? (long long)cnt * zc : zc;       // leading dimension of Z
+  const long long zstep = mergeN ? zc : zsz;                      // offset of Z[b] relative to Z[0]
   {
     HOut z{};
     z.o.C = reinterpret_cast<double*>(zoff); z.c_ws = true;
-    z.o.bsC = zsz; z.o.M = zr; z.o.N = zc; z.o.ldc = zc; z.o.accumulate = 0;
-    z.batch = cnt; z.work = 0;
-    const Mat& A = left_first ? it.X : it.Y;
-    const Mat& B = left_first ? it.Y : it.W;
-    HSeg h = mkseg(A.p + b0 * A.stride, A.ld, A.tr, B.p + b0 * B.stride, B.ld, B.tr, A.cols);
-    h.s.bsA = A.stride; h.s.bsB = B.stride;
+    z.o.bsC = zsz; z.o.M = mergeM ? cnt * zr : zr; z.o.N = mergeN ? cnt * zc : zc; z.o.ldc = (int)zld;
+    z.o.accumulate = 0;
+    z.batch = (mergeM || mergeN) ? 1 : cnt; z.work = 0;
+    HSeg h = mkseg(A1.p + b0 * A1.stride, A1.ld, A1.tr, B1.p + b0 * B1.stride, B1.ld, B1.tr, A1.cols);
+    if (mergeM) {
+      h.s.amr = zr; h.s.ams = A1.stride; h.s.amr_inv = (unsigned)(0x100000000ull / (unsigned)zr) + 1u;
+    } else if (mergeN) {
+      h.s.bnr = zc; h.s.bns = B1.stride; h.s.bnr_inv = (unsigned)(0x100000000ull / (unsigned)zc) + 1u;
+    } else {
+      h.s.bsA = A1.stride; h.s.bsB = B1.stride;
+    }
     z.segs.push_back(h);
     ch.p1.push_back(std::move(z));
   }
@@ -114,17 +145,17 @@ void Planner::add_piece(const Item& it, int b0, int cnt) {
   HOut& o = p2_out(ch, it, b0, cnt, it.X.rows, it.W.cols);
   HSeg h;
   if (left_first) {
-    h = mkseg(reinterpret_cast<const double*>(zoff), zc, false, it.W.p + b0 * it.W.stride, it.W.ld,
+    h = mkseg(reinterpret_cast<const double*>(zoff), (int)zld, false, it.W.p + b0 * it.W.stride, it.W.ld,
               it.W.tr, zc);
     h.a_ws = true;
-    if (batched) { h.s.bsA = zsz; h.s.bsB = it.W.stride; }
-    else { h.s.count = cnt; h.s.rsA = zsz; h.s.rsB = it.W.stride; }
+    if (batched) { h.s.bsA = zstep; h.s.bsB = it.W.stride; }
+    else { h.s.count = cnt; h.s.rsA = zstep; h.s.rsB = it.W.stride; }
   } else {
-    h = mkseg(it.X.p + b0 * it.X.stride, it.X.ld, it.X.tr, reinterpret_cast<const double*>(zoff), zc,
+    h = mkseg(it.X.p + b0 * it.X.stride, it.X.ld, it.X.tr, reinterpret_cast<const double*>(zoff), (int)zld,
               false, zr);
     h.b_ws = true;
-    if (batched) { h.s.bsA = it.X.stride; h.s.bsB = zsz; }
-    else { h.s.count = cnt; h.s.rsA = it.X.stride; h.s.rsB = zsz; }
+    if (batched) { h.s.bsA = it.X.stride; h.s.bsB = zstep; }
+    else { h.s.count = cnt; h.s.rsA = it.X.stride; h.s.rsB = zstep; }
   }
   h.s.alpha = it.alpha;
   o.segs.push_back(h);
@@ -139,16 +170,102 @@ void Planner::finish(Plan* plan, cudaStream_t st) {
   plan->n_products = n_products_;
   if (ws_max_ > 0) plan->workspace.allocate(al_, (size_t)ws_max_);
   double* ws = plan->workspace.p;
+
+  // ---- split-K: heavy outputs are cut into parts along their (segment, repeat) list so that one launch
+  // has several CTAs per SM of comparable length.  Part 0 accumulates into C; the others write partial
+  // sums to scratch, which a reduction kernel folds into C in a fixed order afterwards.
+  struct HRed { RedDesc d; long long p_off; };
+  std::vector<std::vector<HRed>> reds(chunks_.size());
+  long long scratch_max = 0;
+  auto tile_area = [](int M, int N, double* maxarea) {
+    std::vector<std::pair<int, int>> rs, cs;
+    split_dim(M, rs); split_dim(N, cs);
+    double a = 0, mx = 0;
+    for (auto& r : rs) for (auto& c : cs) {
+      double t = (double)GEMM_DIMS[r.second] * GEMM_DIMS[c.second];
+      a += t; mx = std::max(mx, t);
+    }
+    *maxarea = mx;
+    return a;
+  };
+  for (size_t ci = 0; ci < chunks_.size(); ++ci) {
+    std::vector<HOut>& hv = chunks_[ci].p2;
+    double total = 0;
+    std::vector<double> ks(hv.size()), mxa(hv.size());
+    for (size_t i = 0; i < hv.size(); ++i) {
+      double k = 0;
+      for (auto& hs : hv[i].segs) k += (double)hs.s.K * hs.s.count;
+      ks[i] = k;
+      total += k * tile_area(hv[i].o.M, hv[i].o.N, &mxa[i]) * hv[i].batch;
+    }
+    const double wstar = total / (148.0 * 6.0);
+    std::vector<HOut> ex;
+    long long sc_used = 0;
+    for (size_t i = 0; i < hv.size(); ++i) {
+      HOut& h = hv[i];
+      long long units = 0;
+      for (auto& hs : h.segs) units += hs.s.count;
+      int ns = wstar > 0 ? (int)std::ceil(ks[i] * mxa[i] / wstar) : 1;
+      ns = (int)std::min<long long>(std::min(ns, 16), units);
+      if (ns <= 1) { ex.push_back(std::move(h)); continue; }
+      const long long mn = (long long)h.o.M * h.o.N;
+      HRed rd{};
+      rd.d.C = h.o.C; rd.d.bsC = h.o.bsC; rd.d.M = h.o.M; rd.d.N = h.o.N; rd.d.ldc = h.o.ldc;
+      rd.d.nparts = ns - 1; rd.d.batch = h.batch; rd.p_off = sc_used;
+      reds[ci].push_back(rd);
+      const double target = ks[i] / ns;
+      size_t si = 0; int rep = 0;      // cursor into the (segment, repeat) list
+      for (int p = 0; p < ns; ++p) {
+        HOut part{};
+        part.o = h.o; part.c_ws = false; part.batch = h.batch; part.work = 0;
+        if (p > 0) {
+          part.c_sc = true;
+          part.o.C = reinterpret_cast<double*>(sc_used + (long long)(p - 1) * h.batch * mn);
+          part.o.bsC = mn; part.o.ldc = h.o.N; part.o.accumulate = 0;
+        }
+        double got = 0;
+        while (si < h.segs.size() && (p == ns - 1 || got < target)) {
+          const HSeg& hs = h.segs[si];
+          const int left = hs.s.count - rep;
+          int take = left;
+          if (p != ns - 1) {
+            double room = target - got;
+            take = (int)std::min<double>(left, std::max(1.0, std::floor(room / hs.s.K + 0.5)));
+          }
+          HSeg sub = hs;
+          sub.s.count = take;
+          if (rep > 0) {
+            if (hs.a_ws) sub.s.A = reinterpret_cast<const double*>(reinterpret_cast<long long>(hs.s.A) + rep * hs.s.rsA);
+            else sub.s.A = hs.s.A + rep * hs.s.rsA;
+            if (hs.b_ws) sub.s.B = reinterpret_cast<const double*>(reinterpret_cast<long long>(hs.s.B) + rep * hs.s.rsB);
+            else sub.s.B = hs.s.B + rep * hs.s.rsB;
+          }
+          part.segs.push_back(sub);
+          got += (double)take * hs.s.K;
+          rep += take;
+          if (rep >= hs.s.count) { rep = 0; ++si; }
+        }
+        if (!part.segs.empty() || p == 0) ex.push_back(std::move(part));
+        else reds[ci].back().d.nparts = std::min(reds[ci].back().d.nparts, p - 1);
+      }
+      sc_used += (long long)(ns - 1) * h.batch * mn;
+    }
+    hv.swap(ex);
+    scratch_max = std::max(scratch_max, sc_used);
+  }
+  if (scratch_max > 0) plan->scratch.allocate(al_, (size_t)scratch_max);
+  double* sc = plan->scratch.p;
   auto build = [&](std::vector<HOut>& hv, Phase& ph) {
     std::vector<GOut> outs;
     std::vector<GSeg> segs;
     struct TW { GTile t; double w; };
-    std::vector<TW> tw;
+    std::vector<TW> tw[GEMM_NSHAPES];
     outs.reserve(hv.size());
     for (size_t oi = 0; oi < hv.size(); ++oi) {
       HOut& h = hv[oi];
       GOut o = h.o;
       if (h.c_ws) o.C = ws + reinterpret_cast<long long>(h.o.C);
+      if (h.c_sc) o.C = sc + reinterpret_cast<long long>(h.o.C);
       o.seg_begin = (int)segs.size();
       double ksum = 0;
       for (auto& hs : h.segs) {
@@ -159,32 +276,46 @@ void Planner::finish(Plan* plan, cudaStream_t st) {
         segs.push_back(s);
       }
       o.seg_end = (int)segs.size();
-      int tm = (o.M + GEMM_BM - 1) / GEMM_BM, tn = (o.N + GEMM_BN - 1) / GEMM_BN;
-      o.tile_m = pad8((o.M + tm - 1) / tm);
-      o.tile_n = pad8((o.N + tn - 1) / tn);
-      tm = (o.M + o.tile_m - 1) / o.tile_m;
-      tn = (o.N + o.tile_n - 1) / o.tile_n;
       outs.push_back(o);
+      std::vector<std::pair<int, int>> rs, cs;
+      split_dim(o.M, rs);
+      split_dim(o.N, cs);
       for (int b = 0; b < h.batch; ++b)
-        for (int i = 0; i < tm; ++i)
-          for (int j = 0; j < tn; ++j) {
-            int em = std::min(o.tile_m, o.M - i * o.tile_m), en = std::min(o.tile_n, o.N - j * o.tile_n);
-            double w = ksum * ((em + 15) / 16) * ((en + 31) / 32);
-            tw.push_back({GTile{(int)oi, b, i, j}, w});
+        for (auto& r : rs)
+          for (auto& c : cs) {
+            int shape = 3 * r.second + c.second;
+            double w = ksum * GEMM_DIMS[r.second] * GEMM_DIMS[c.second];
+            tw[shape].push_back({GTile{(int)oi, b, r.first, c.first}, w});
           }
     }
-    std::stable_sort(tw.begin(), tw.end(), [](const TW& a, const TW& b) { return a.w > b.w; });
-    std::vector<GTile> tiles(tw.size());
-    for (size_t i = 0; i < tw.size(); ++i) tiles[i] = tw[i].t;
-    ph.ntiles = (int)tiles.size();
+    for (int s = 0; s < GEMM_NSHAPES; ++s) {
+      std::stable_sort(tw[s].begin(), tw[s].end(), [](const TW& a, const TW& b) { return a.w > b.w; });
+      std::vector<GTile> tiles(tw[s].size());
+      for (size_t i = 0; i < tw[s].size(); ++i) tiles[i] = tw[s][i].t;
+      ph.ntiles[s] = (int)tiles.size();
+      if (!tiles.empty()) ph.tiles[s].upload(al_, tiles, st);
+    }
     ph.outs.upload(al_, outs, st);
     ph.segs.upload(al_, segs, st);
-    ph.tiles.upload(al_, tiles, st);
   };
   plan->chunks.resize(chunks_.size());
   for (size_t c = 0; c < chunks_.size(); ++c) {
     build(chunks_[c].p1, plan->chunks[c].p1);
     build(chunks_[c].p2, plan->chunks[c].p2);
+    if (!reds[c].empty()) {
+      std::vector<RedDesc> rd;
+      int mb = 1;
+      for (auto& r : reds[c]) {
+        if (r.d.nparts <= 0) continue;
+        RedDesc d = r.d;
+        d.P = sc + r.p_off;
+        mb = std::max(mb, d.batch);
+        rd.push_back(d);
+      }
+      plan->chunks[c].p2.nred = (int)rd.size();
+      plan->chunks[c].p2.red_max_batch = mb;
+      if (!rd.empty()) plan->chunks[c].p2.red.upload(al_, rd, st);
+    }
   }
   chunks_.clear();
 }

@@ -13,6 +13,7 @@
 
 #include "common.h"
 #include "gemm.cuh"
+#include "kernels.cuh"
 
 namespace dmrg {
 
@@ -40,8 +41,11 @@ struct Item {
 struct Phase {
   DevArray<GOut> outs;
   DevArray<GSeg> segs;
-  DevArray<GTile> tiles;
-  int ntiles = 0;
+  DevArray<GTile> tiles[GEMM_NSHAPES];   // one tile list per tile shape, heaviest tiles first
+  int ntiles[GEMM_NSHAPES] = {0, 0, 0, 0, 0, 0, 0, 0, 0};
+  DevArray<RedDesc> red;                  // split-K partial sums to fold into the outputs afterwards
+  int nred = 0, red_max_batch = 1;
+  int launches() const { int n = nred > 0; for (int s = 0; s < GEMM_NSHAPES; ++s) n += ntiles[s] > 0; return n; }
 };
 
 struct Chunk {
@@ -50,12 +54,12 @@ struct Chunk {
 
 struct Plan {
   std::vector<Chunk> chunks;
-  DevArray<double> workspace;
+  DevArray<double> workspace, scratch;
   double flops_analytic = 0, flops_executed = 0, bytes_intermediate = 0;
   int64_t n_items = 0, n_products = 0;
   int launches() const;
   void run(cudaStream_t st, int64_t* launch_counter) const;
-  void clear() { chunks.clear(); workspace.release(); }
+  void clear() { chunks.clear(); workspace.release(); scratch.release(); }
 };
 
 class Planner {
@@ -67,7 +71,7 @@ class Planner {
 
  private:
   struct HSeg { GSeg s; bool a_ws, b_ws; };          // *_ws: pointer is a workspace offset
-  struct HOut { GOut o; bool c_ws; std::vector<HSeg> segs; int batch; double work; };
+  struct HOut { GOut o; bool c_ws; std::vector<HSeg> segs; int batch; double work; bool c_sc = false; };
   struct HChunk {
     std::vector<HOut> p1;
     std::vector<HOut> p2;
