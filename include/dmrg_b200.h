@@ -156,6 +156,19 @@ int dmrg_env_export(dmrg_ctx* ctx, int32_t side, int32_t kind, int32_t i, int32_
  * SMs, timed with CUDA events on `stream`. */
 int dmrg_fp64_peak(dmrg_ctx* ctx, double* h_tflops, void* stream);
 
+/* Per-launch timing of one H_eff.psi (measurement aid): runs dmrg_heff_apply with every
+ * kernel launch of the task plan bracketed by CUDA events on `stream` and synchronises.  Up to `cap`
+ * records are written to h_out; *n receives the number of launches.  phase 1 = O_L.psi (or psi.O_R^T)
+ * into the workspace, phase 2 = accumulation into psi'; shape = tile shape index 3*row_class+col_class
+ * with classes {32,64,128}, -1 = split-K reduction; flops = flops the launch's tiles execute. */
+typedef struct {
+  int32_t chunk, phase, shape, ntiles;
+  double flops;
+  double ms;
+} dmrg_launch_info;
+int dmrg_apply_profile(dmrg_ctx* ctx, const double* d_psi_in, double* d_psi_out, int32_t cap,
+                       dmrg_launch_info* h_out, int32_t* n, void* stream);
+
 #ifdef __cplusplus
 }
 #endif

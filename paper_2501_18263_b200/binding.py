@@ -21,7 +21,7 @@ EXPORTS = [
     "dmrg_create", "dmrg_destroy", "dmrg_last_error", "dmrg_load_integrals", "dmrg_mps_set_sectors",
     "dmrg_mps_set_site", "dmrg_env_build", "dmrg_renormalize", "dmrg_psi_layout", "dmrg_heff_apply",
     "dmrg_heff_diag", "dmrg_davidson", "dmrg_heff_apply_host", "dmrg_davidson_host", "dmrg_stats",
-    "dmrg_env_export", "dmrg_fp64_peak",
+    "dmrg_env_export", "dmrg_fp64_peak", "dmrg_apply_profile",
 ]
 
 ALLOC_FN = C.CFUNCTYPE(C.c_void_p, C.c_uint64, C.c_void_p)
@@ -49,6 +49,11 @@ class Stats(C.Structure):
 
     def as_dict(self):
         return {f: getattr(self, f) for f, _ in self._fields_}
+
+
+class LaunchInfo(C.Structure):
+    _fields_ = [("chunk", C.c_int32), ("phase", C.c_int32), ("shape", C.c_int32), ("ntiles", C.c_int32),
+                ("flops", C.c_double), ("ms", C.c_double)]
 
 
 _lib = None
@@ -83,6 +88,7 @@ def load_library(build_if_missing: bool = True):
     lib.dmrg_stats.argtypes = [vp, C.POINTER(Stats)]
     lib.dmrg_env_export.argtypes = [vp, i32, i32, i32, i32, vp, C.POINTER(i64)]
     lib.dmrg_fp64_peak.argtypes = [vp, dp, vp]
+    lib.dmrg_apply_profile.argtypes = [vp, vp, vp, i32, C.POINTER(LaunchInfo), C.POINTER(i32), vp]
     for name in EXPORTS:
         if name != "dmrg_last_error":
             getattr(lib, name).restype = C.c_int
@@ -254,6 +260,15 @@ class DMRG:
         v = C.c_double()
         self._check(self.lib.dmrg_fp64_peak(self.ctx, C.byref(v), self._stream()))
         return v.value
+
+    def apply_profile(self, psi_in, psi_out=None, cap=4096):
+        """One H_eff.psi with per-launch event timing; returns (psi_out, list of dict per launch)."""
+        if psi_out is None:
+            psi_out = self.torch.empty_like(psi_in)
+        arr, n = (LaunchInfo * cap)(), C.c_int32()
+        self._check(self.lib.dmrg_apply_profile(self.ctx, C.c_void_p(psi_in.data_ptr()), C.c_void_p(psi_out.data_ptr()),
+                                                cap, arr, C.byref(n), self._stream()))
+        return psi_out, [{f: getattr(arr[i], f) for f, _ in LaunchInfo._fields_} for i in range(min(n.value, cap))]
 
     # -- convenience: load everything a two-site problem needs from the generator objects --
     def setup(self, T, V, mps, e_core=0.0):

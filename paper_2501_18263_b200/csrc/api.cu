@@ -501,6 +501,24 @@ int dmrg_env_export(dmrg_ctx* ctx, int32_t side, int32_t kind, int32_t i, int32_
   API_END
 }
 
+int dmrg_apply_profile(dmrg_ctx* ctx, const double* d_in, double* d_out, int32_t cap, dmrg_launch_info* h_out,
+                       int32_t* n, void* stream) {
+  API_BEGIN
+  cudaStream_t st = (cudaStream_t)stream;
+  DMRG_REQUIRE(ctx->k > 0 && d_in && d_out && n, DMRG_ERR_ARG, "apply_profile: bad arguments");
+  launch_pack(ctx->d_psi_blocks.p, (int)ctx->psi.size(), d_in, ctx->psi_in_p.p, st);
+  DMRG_CUDA(cudaMemsetAsync(ctx->psi_out_p.p, 0, (size_t)ctx->psi_np * 8, st));
+  std::vector<LaunchRecord> rec;
+  ctx->apply_plan.run_profiled(st, &rec);
+  launch_unpack(ctx->d_psi_blocks.p, (int)ctx->psi.size(), ctx->psi_out_p.p, d_out, ctx->e_core, d_in, st);
+  ctx->launches += 3 + (int64_t)rec.size();
+  DMRG_CUDA(cudaStreamSynchronize(st));
+  *n = (int32_t)rec.size();
+  for (int i = 0; i < (int)rec.size() && i < cap && h_out; ++i)
+    h_out[i] = dmrg_launch_info{rec[i].chunk, rec[i].phase, rec[i].shape, rec[i].ntiles, rec[i].flops, (double)rec[i].ms};
+  API_END
+}
+
 int dmrg_fp64_peak(dmrg_ctx* ctx, double* h_tflops, void* stream) {
   API_BEGIN
   DMRG_REQUIRE(h_tflops, DMRG_ERR_ARG, "fp64_peak: null pointer");

@@ -30,6 +30,36 @@ void Plan::run(cudaStream_t st, int64_t* launch_counter) const {
   }
 }
 
+void Plan::run_profiled(cudaStream_t st, std::vector<LaunchRecord>* out) const {
+  std::vector<cudaEvent_t> ev;
+  auto mark = [&]() {
+    cudaEvent_t e;
+    DMRG_CUDA(cudaEventCreate(&e));
+    DMRG_CUDA(cudaEventRecord(e, st));
+    ev.push_back(e);
+  };
+  out->clear();
+  mark();
+  for (size_t c = 0; c < chunks.size(); ++c)
+    for (int p = 0; p < 2; ++p) {
+      const Phase& ph = p == 0 ? chunks[c].p1 : chunks[c].p2;
+      for (int s = GEMM_NSHAPES - 1; s >= 0; --s) {
+        if (ph.ntiles[s] <= 0) continue;
+        DMRG_CUDA(launch_grouped_gemm(s, ph.outs.p, ph.segs.p, ph.tiles[s].p, ph.ntiles[s], st));
+        mark();
+        out->push_back(LaunchRecord{(int)c, p + 1, s, ph.ntiles[s], ph.shape_flops[s], 0.f});
+      }
+      if (ph.nred > 0) {
+        launch_reduce_partials(ph.red.p, ph.nred, ph.red_max_batch, st);
+        mark();
+        out->push_back(LaunchRecord{(int)c, p + 1, -1, ph.nred, 0.0, 0.f});
+      }
+    }
+  DMRG_CUDA(cudaStreamSynchronize(st));
+  for (size_t i = 0; i < out->size(); ++i) DMRG_CUDA(cudaEventElapsedTime(&(*out)[i].ms, ev[i], ev[i + 1]));
+  for (auto e : ev) cudaEventDestroy(e);
+}
+
 static inline double fl(double a, double b, double c) { return 2.0 * a * b * c; }
 
 // Splits an extent (multiple of 8) into tile rows/cols of class 0/1/2 = 32/64/128: (start, class).
@@ -286,6 +316,8 @@ void Planner::finish(Plan* plan, cudaStream_t st) {
             int shape = 3 * r.second + c.second;
             double w = ksum * GEMM_DIMS[r.second] * GEMM_DIMS[c.second];
             tw[shape].push_back({GTile{(int)oi, b, r.first, c.first}, w});
+            ph.shape_flops[shape] += 2.0 * ksum * std::min(GEMM_DIMS[r.second], o.M - r.first) *
+                                     std::min(GEMM_DIMS[c.second], o.N - c.first);
           }
     }
     for (int s = 0; s < GEMM_NSHAPES; ++s) {

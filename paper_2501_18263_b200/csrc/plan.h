@@ -43,6 +43,7 @@ struct Phase {
   DevArray<GSeg> segs;
   DevArray<GTile> tiles[GEMM_NSHAPES];   // one tile list per tile shape, heaviest tiles first
   int ntiles[GEMM_NSHAPES] = {0, 0, 0, 0, 0, 0, 0, 0, 0};
+  double shape_flops[GEMM_NSHAPES] = {0, 0, 0, 0, 0, 0, 0, 0, 0};   // flops the tiles of each launch execute
   DevArray<RedDesc> red;                  // split-K partial sums to fold into the outputs afterwards
   int nred = 0, red_max_batch = 1;
   int launches() const { int n = nred > 0; for (int s = 0; s < GEMM_NSHAPES; ++s) n += ntiles[s] > 0; return n; }
@@ -52,6 +53,9 @@ struct Chunk {
   Phase p1, p2;
 };
 
+// One kernel launch of a plan, timed with CUDA events (dmrg_apply_profile).
+struct LaunchRecord { int chunk, phase, shape, ntiles; double flops; float ms; };
+
 struct Plan {
   std::vector<Chunk> chunks;
   DevArray<double> workspace, scratch;
@@ -59,6 +63,8 @@ struct Plan {
   int64_t n_items = 0, n_products = 0;
   int launches() const;
   void run(cudaStream_t st, int64_t* launch_counter) const;
+  // Same launches, each bracketed by events (shape -1 = split-K reduction).  Synchronises `st`.
+  void run_profiled(cudaStream_t st, std::vector<LaunchRecord>* out) const;
   void clear() { chunks.clear(); workspace.release(); scratch.release(); }
 };
 
