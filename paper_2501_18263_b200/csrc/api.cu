@@ -4,6 +4,7 @@
 #include <algorithm>
 #include <chrono>
 #include <cmath>
+#include <cstdlib>
 #include <cstring>
 
 #include "engine.h"
@@ -44,6 +45,12 @@ int dmrg_create(const dmrg_config* cfg, dmrg_ctx** out) {
   c->al.user = cfg->alloc_user;
   c->L = cfg->L;
   c->site.resize(cfg->L + 2);
+  try {
+    if (!std::getenv("DMRG_B200_SERIAL")) c->exec.init();   // debugging aid: every launch in order on one stream
+  } catch (const dmrg::Error&) {
+    delete c;
+    return DMRG_ERR_CUDA;
+  }
   *out = c;
   return DMRG_OK;
 }
@@ -253,7 +260,7 @@ int dmrg_psi_layout(dmrg_ctx* ctx, int32_t* nblocks, dmrg_psi_block* out, int64_
 static void apply_padded(dmrg_ctx* ctx, cudaStream_t st) {
   DMRG_CUDA(cudaMemsetAsync(ctx->psi_out_p.p, 0, (size_t)ctx->psi_np * 8, st));
   ++ctx->launches;
-  ctx->apply_plan.run(st, &ctx->launches);
+  ctx->apply_plan.run(st, &ctx->launches, ctx->ex());
 }
 
 int dmrg_heff_apply(dmrg_ctx* ctx, const double* d_in, double* d_out, void* stream) {

@@ -225,7 +225,7 @@ struct Presummer {
   void run() {
     Plan p;
     planner.finish(&p, st);
-    p.run(st, &ctx->launches);
+    p.run(st, &ctx->launches, ctx->ex());
     DMRG_CUDA(cudaStreamSynchronize(st));
     coefs.clear();
   }
@@ -485,7 +485,7 @@ std::unique_ptr<BlockSide> renormalize_block(dmrg_ctx* ctx, const BlockSide& old
   }
   Plan plan;
   planner.finish(&plan, st);
-  plan.run(st, &ctx->launches);
+  plan.run(st, &ctx->launches, ctx->ex());
   DMRG_CUDA(cudaStreamSynchronize(st));
   if (flops_out) *flops_out = plan.flops_analytic;
   return nb;

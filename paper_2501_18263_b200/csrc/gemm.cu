@@ -1,4 +1,4 @@
-// Grouped FP64 GEMM kernels: one CTA per output tile, 8 warps, DMMA m8n8k4, multi-stage cp.async
+// Grouped FP64 GEMM kernels: one CTA per output tile, 8 or 16 warps, DMMA m8n8k4, multi-stage cp.async
 // pipeline that runs across segment boundaries.  Nine tile shapes ({32,64,128}^2) are instantiated;
 // the inner loop is branch-free with compile-time shared-memory offsets for each of the four
 // operand-layout combinations.  See gemm.cuh for the contract.
@@ -10,7 +10,6 @@ namespace {
 
 constexpr int KC = 16;        // K extent of one pipeline stage
 constexpr int PK = KC + 4;    // pitch of the K-contiguous tile format [x][k]   (conflict-free LDS.64)
-constexpr int NT = 256;       // threads per CTA
 
 __device__ __forceinline__ void cp_async16(void* smem, const void* gmem) {
   unsigned s = static_cast<unsigned>(__cvta_generic_to_shared(smem));
@@ -71,7 +70,7 @@ __device__ __forceinline__ long long seg_off(int x, int nr, unsigned inv, long l
 // Copy one operand tile into shared memory.  BX = tile extent in the non-K dimension.
 //   xcontig == 0: element (x, k) at src[x*ld + k]  -> smem [x][k], pitch PK
 //   xcontig == 1: element (x, k) at src[k*ld + x]  -> smem [k][x], pitch BX + 4
-template <int BX>
+template <int BX, int NT>
 __device__ __forceinline__ void load_tile(double* sm, const double* base, int ld, int x0, int ext, int k0,
                                           int kv, int xcontig, int nr, unsigned inv, long long stride, int tid) {
   constexpr int ITERS = (BX * KC / 2) / NT;
@@ -131,9 +130,9 @@ __device__ __forceinline__ void compute_stage(double (&acc)[FA][FB][2], const do
 }
 
 template <int BM, int BN, int WR, int WC, int STAGES, int MINB>
-__global__ void __launch_bounds__(NT, MINB)
+__global__ void __launch_bounds__(32 * WR * WC, MINB)
 k_grouped_gemm(const GOut* __restrict__ outs, const GSeg* __restrict__ segs, const GTile* __restrict__ tiles) {
-  static_assert(WR * WC == 8, "eight warps per CTA");
+  constexpr int NT = 32 * WR * WC;   // threads per CTA
   constexpr int WM = BM / WR, WN = BN / WC, FA = WM / 8, FB = WN / 8;
   constexpr int TA = BM * PK, TB = BN * PK, STAGE = TA + TB;
   extern __shared__ __align__(16) double smem[];
@@ -162,10 +161,10 @@ k_grouped_gemm(const GOut* __restrict__ outs, const GSeg* __restrict__ segs, con
       const int kv = min(KC, prod.K - prod.k0);
       const int ta = prod.flags & 1, tb = (prod.flags >> 1) & 1;
       // op(A)(m,k): !ta -> A[m*lda+k] (K-contig) ; ta -> A[k*lda+m] (X-contig)
-      load_tile<BM>(sA, prod.A + prod.rep * prod.rsA, prod.lda, m0, em, prod.k0, kv, ta, prod.amr,
+      load_tile<BM, NT>(sA, prod.A + prod.rep * prod.rsA, prod.lda, m0, em, prod.k0, kv, ta, prod.amr,
                     prod.amr_inv, prod.ams, tid);
       // op(B)(k,n): !tb -> B[k*ldb+n] (X-contig) ; tb -> B[n*ldb+k] (K-contig)
-      load_tile<BN>(sB, prod.B + prod.rep * prod.rsB, prod.ldb, n0, en, prod.k0, kv, !tb, prod.bnr,
+      load_tile<BN, NT>(sB, prod.B + prod.rep * prod.rsB, prod.ldb, n0, en, prod.k0, kv, !tb, prod.bnr,
                     prod.bnr_inv, prod.bns, tid);
       prod.next();
     }
@@ -230,7 +229,7 @@ struct Cfg {
                                 cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
   }
   static cudaError_t launch(const GOut* o, const GSeg* s, const GTile* t, int n, cudaStream_t st) {
-    k_grouped_gemm<BM, BN, WR, WC, STAGES, MINB><<<n, NT, smem, st>>>(o, s, t);
+    k_grouped_gemm<BM, BN, WR, WC, STAGES, MINB><<<n, 32 * WR * WC, smem, st>>>(o, s, t);
     return cudaGetLastError();
   }
 };
@@ -244,7 +243,7 @@ using S64x64   = Cfg<64, 64, 2, 4, 3, 3>;
 using S64x128  = Cfg<64, 128, 2, 4, 3, 2>;
 using S128x32  = Cfg<128, 32, 8, 1, 3, 3>;
 using S128x64  = Cfg<128, 64, 4, 2, 3, 2>;
-using S128x128 = Cfg<128, 128, 2, 4, 4, 1>;
+using S128x128 = Cfg<128, 128, 4, 4, 4, 1>;
 
 }  // namespace
 

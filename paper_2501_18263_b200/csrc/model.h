@@ -111,6 +111,8 @@ struct dmrg_ctx {
   dmrg::DevArray<dmrg::PsiBlockDev> d_psi_blocks;
   dmrg::DevArray<double> psi_in_p, psi_out_p, diag_p;
   dmrg::Plan apply_plan;
+  dmrg::Exec exec;                              // worker streams (plan.h)
+  dmrg::Exec* ex() { return exec.ok ? &exec : nullptr; }
   dmrg_stats_t stats{};
   int64_t launches = 0;
   // Davidson workspace

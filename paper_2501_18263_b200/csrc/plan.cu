@@ -11,22 +11,60 @@ int Plan::launches() const {
   return n;
 }
 
-static void run_phase(const Phase& ph, cudaStream_t st, int64_t* launch_counter) {
-  for (int s = GEMM_NSHAPES - 1; s >= 0; --s) {   // largest tiles first
-    if (ph.ntiles[s] <= 0) continue;
-    DMRG_CUDA(launch_grouped_gemm(s, ph.outs.p, ph.segs.p, ph.tiles[s].p, ph.ntiles[s], st));
-    if (launch_counter) ++*launch_counter;
+void Exec::init() {
+  if (ok) return;
+  for (int i = 0; i < NW; ++i) {
+    DMRG_CUDA(cudaStreamCreateWithFlags(&w[i], cudaStreamNonBlocking));
+    DMRG_CUDA(cudaEventCreateWithFlags(&join[i], cudaEventDisableTiming));
   }
-  if (ph.nred > 0) {
-    launch_reduce_partials(ph.red.p, ph.nred, ph.red_max_batch, st);
-    if (launch_counter) ++*launch_counter;
-  }
+  DMRG_CUDA(cudaEventCreateWithFlags(&fork, cudaEventDisableTiming));
+  ok = true;
+}
+Exec::~Exec() {
+  if (!ok) return;
+  for (int i = 0; i < NW; ++i) { cudaStreamDestroy(w[i]); cudaEventDestroy(join[i]); }
+  cudaEventDestroy(fork);
 }
 
-void Plan::run(cudaStream_t st, int64_t* launch_counter) const {
-  for (const auto& c : chunks) {
-    run_phase(c.p1, st, launch_counter);
-    run_phase(c.p2, st, launch_counter);
+namespace {
+struct Launch { const Phase* ph; int shape; double work; };
+void collect(const Phase& ph, std::vector<Launch>& v) {
+  for (int s = GEMM_NSHAPES - 1; s >= 0; --s)
+    if (ph.ntiles[s] > 0) v.push_back(Launch{&ph, s, ph.shape_flops[s]});
+}
+}  // namespace
+
+void Plan::run(cudaStream_t st, int64_t* launch_counter, Exec* ex) const {
+  const int n = (int)chunks.size();
+  for (int stage = 0; stage <= n; ++stage) {
+    std::vector<Launch> ls;
+    if (stage > 0) collect(chunks[stage - 1].p2, ls);
+    if (stage < n) collect(chunks[stage].p1, ls);
+    if (ls.empty()) continue;
+    if (launch_counter) *launch_counter += (int64_t)ls.size();
+    if (!ex || ls.size() == 1) {
+      for (auto& l : ls)
+        DMRG_CUDA(launch_grouped_gemm(l.shape, l.ph->outs.p, l.ph->segs.p, l.ph->tiles[l.shape].p, l.ph->ntiles[l.shape], st));
+    } else {
+      std::stable_sort(ls.begin(), ls.end(), [](const Launch& a, const Launch& b) { return a.work > b.work; });
+      DMRG_CUDA(cudaEventRecord(ex->fork, st));
+      const int nw = std::min<int>(Exec::NW, (int)ls.size());
+      for (int i = 0; i < nw; ++i) DMRG_CUDA(cudaStreamWaitEvent(ex->w[i], ex->fork, 0));
+      for (size_t i = 0; i < ls.size(); ++i) {
+        const Launch& l = ls[i];
+        DMRG_CUDA(launch_grouped_gemm(l.shape, l.ph->outs.p, l.ph->segs.p, l.ph->tiles[l.shape].p, l.ph->ntiles[l.shape],
+                                      ex->w[i % nw]));
+      }
+      for (int i = 0; i < nw; ++i) {
+        DMRG_CUDA(cudaEventRecord(ex->join[i], ex->w[i]));
+        DMRG_CUDA(cudaStreamWaitEvent(st, ex->join[i], 0));
+      }
+    }
+    if (stage > 0 && chunks[stage - 1].p2.nred > 0) {
+      const Phase& ph = chunks[stage - 1].p2;
+      launch_reduce_partials(ph.red.p, ph.nred, ph.red_max_batch, st);
+      if (launch_counter) ++*launch_counter;
+    }
   }
 }
 
@@ -198,7 +236,9 @@ void Planner::finish(Plan* plan, cudaStream_t st) {
   plan->bytes_intermediate = bi_;
   plan->n_items = n_items_;
   plan->n_products = n_products_;
-  if (ws_max_ > 0) plan->workspace.allocate(al_, (size_t)ws_max_);
+  const bool two_halves = chunks_.size() > 1;
+  plan->ws_half = ws_max_;
+  if (ws_max_ > 0) plan->workspace.allocate(al_, (size_t)ws_max_ * (two_halves ? 2 : 1));
   double* ws = plan->workspace.p;
 
   // ---- split-K: heavy outputs are cut into parts along their (segment, repeat) list so that one launch
@@ -285,7 +325,7 @@ void Planner::finish(Plan* plan, cudaStream_t st) {
   }
   if (scratch_max > 0) plan->scratch.allocate(al_, (size_t)scratch_max);
   double* sc = plan->scratch.p;
-  auto build = [&](std::vector<HOut>& hv, Phase& ph) {
+  auto build = [&](std::vector<HOut>& hv, Phase& ph, double* ws) {
     std::vector<GOut> outs;
     std::vector<GSeg> segs;
     struct TW { GTile t; double w; };
@@ -332,8 +372,9 @@ void Planner::finish(Plan* plan, cudaStream_t st) {
   };
   plan->chunks.resize(chunks_.size());
   for (size_t c = 0; c < chunks_.size(); ++c) {
-    build(chunks_[c].p1, plan->chunks[c].p1);
-    build(chunks_[c].p2, plan->chunks[c].p2);
+    double* wsc = ws + ((c & 1) ? ws_max_ : 0);   // chunk c works in workspace half c & 1
+    build(chunks_[c].p1, plan->chunks[c].p1, wsc);
+    build(chunks_[c].p2, plan->chunks[c].p2, wsc);
     if (!reds[c].empty()) {
       std::vector<RedDesc> rd;
       int mb = 1;

@@ -53,16 +53,32 @@ struct Chunk {
   Phase p1, p2;
 };
 
+// Worker streams for running the independent launches of a plan stage concurrently (fork/join with
+// events around the caller's stream).  Kernels of different tile shapes have very different grid
+// sizes; run back to back each one ends in its own under-filled tail, run side by side they fill it.
+struct Exec {
+  static constexpr int NW = 6;
+  cudaStream_t w[NW] = {};
+  cudaEvent_t fork = nullptr, join[NW] = {};
+  bool ok = false;
+  void init();
+  ~Exec();
+};
+
 // One kernel launch of a plan, timed with CUDA events (dmrg_apply_profile).
 struct LaunchRecord { int chunk, phase, shape, ntiles; double flops; float ms; };
 
 struct Plan {
   std::vector<Chunk> chunks;
   DevArray<double> workspace, scratch;
+  long long ws_half = 0;   // elements per workspace half (two halves when there are several chunks)
   double flops_analytic = 0, flops_executed = 0, bytes_intermediate = 0;
   int64_t n_items = 0, n_products = 0;
   int launches() const;
-  void run(cudaStream_t st, int64_t* launch_counter) const;
+  // Stages: P1(0) | P2(c-1) + P1(c) ... | P2(last); the launches of a stage are independent (phase 1 of
+  // chunk c writes workspace half c&1 while phase 2 of chunk c-1 reads the other half) and run on the
+  // worker streams of `ex` (nullptr: everything in order on `st`).
+  void run(cudaStream_t st, int64_t* launch_counter, Exec* ex = nullptr) const;
   // Same launches, each bracketed by events (shape -1 = split-K reduction).  Synchronises `st`.
   void run_profiled(cudaStream_t st, std::vector<LaunchRecord>* out) const;
   void clear() { chunks.clear(); workspace.release(); scratch.release(); }
@@ -70,7 +86,8 @@ struct Plan {
 
 class Planner {
  public:
-  Planner(Allocator* al, uint64_t workspace_cap_bytes) : al_(al), cap_(workspace_cap_bytes / 8) {}
+  // A chunk may use half the cap: consecutive chunks alternate between two workspace halves.
+  Planner(Allocator* al, uint64_t workspace_cap_bytes) : al_(al), cap_(workspace_cap_bytes / 16) {}
   void add(const Item& it);
   // Uploads descriptors, allocates the workspace and patches workspace-relative pointers.
   void finish(Plan* plan, cudaStream_t st);
