@@ -280,7 +280,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=3)
     ap.add_argument("--D", type=int, default=0)
-    ap.add_argument("--workspace-gb", type=int, default=16, dest="workspace_gb")
+    ap.add_argument("--workspace-gb", type=int, default=0, dest="workspace_gb", help="0 = library default")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--quick", action="store_true", help="skip the Davidson / renormalisation extras")
     args = ap.parse_args()

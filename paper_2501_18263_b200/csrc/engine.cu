@@ -268,6 +268,16 @@ std::unique_ptr<BlockSide> vacuum_block(dmrg_ctx* ctx, bool is_left, cudaStream_
   return B;
 }
 
+// Workspace cap for the O_L.psi intermediates: the caller's, else a third of the free device memory
+// (1..64 GB).  Fewer, larger chunks mean fewer under-filled launch tails per apply.
+static uint64_t workspace_cap(const dmrg_ctx* ctx) {
+  if (ctx->cfg.workspace_bytes) return ctx->cfg.workspace_bytes;
+  size_t fr = 0, tot = 0;
+  if (cudaMemGetInfo(&fr, &tot) != cudaSuccess) return 16ull << 30;
+  uint64_t cap = fr / 3;
+  return std::min<uint64_t>(std::max<uint64_t>(cap, 1ull << 30), 64ull << 30);
+}
+
 static inline uint64_t pack_key(int a, int b, int c, int d, int e, int f) {
   return ((uint64_t)a << 40) | ((uint64_t)b << 28) | ((uint64_t)c << 22) | ((uint64_t)d << 10) |
          ((uint64_t)e << 9) | (uint64_t)f;
@@ -428,7 +438,7 @@ std::unique_ptr<BlockSide> renormalize_block(dmrg_ctx* ctx, const BlockSide& old
     for (auto& r : make_runs(f.e)) { cuts[f.g.dk].insert(r.a0); cuts[f.g.dk].insert(r.a0 + r.cnt); }
 
   // ---- emit the triple products  new(q2' <- q1') += alpha * W2^T op(S)(q2 <- q1) W1 ----
-  const uint64_t cap = ctx->cfg.workspace_bytes ? ctx->cfg.workspace_bytes : (16ull << 30);
+  const uint64_t cap = workspace_cap(ctx);
   Planner planner(&ctx->al, cap);
   for (auto& f : fgs) {
     OpClass& D = *B.cls[f.g.dk];
@@ -665,7 +675,7 @@ void prepare_superblock(dmrg_ctx* ctx, cudaStream_t st) {
   pre.run();
 
   // ---- tasks of PAPER.md Eq. (8): (term group x psi block) -> contraction items + diagonal tasks ----
-  const uint64_t cap = ctx->cfg.workspace_bytes ? ctx->cfg.workspace_bytes : (16ull << 30);
+  const uint64_t cap = workspace_cap(ctx);
   Planner planner(&ctx->al, cap);
   std::vector<std::vector<DiagTask>> dtasks(ctx->psi.size());
   int64_t n_tasks = 0, n_groups = 0;

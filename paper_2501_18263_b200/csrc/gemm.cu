@@ -1,7 +1,19 @@
-// Grouped FP64 GEMM kernels: one CTA per output tile, 8 or 16 warps, DMMA m8n8k4, multi-stage cp.async
-// pipeline that runs across segment boundaries.  Nine tile shapes ({32,64,128}^2) are instantiated;
-// the inner loop is branch-free with compile-time shared-memory offsets for each of the four
-// operand-layout combinations.  See gemm.cuh for the contract.
+// Grouped FP64 GEMM kernels (sm_100a): warp-specialised, NP producer warps + WR*WC consumer warps.
+//
+//   producer warps: walk the (segment, repeat, k-chunk) list of the CTA's output tiles and stream the two
+//                   operand tiles of every k-chunk into a ring of shared-memory stages with 16-byte
+//                   cp.async copies whose completion is counted on the stage's "full" mbarrier
+//                   (cp.async.mbarrier.arrive.noinc).  They never wait for the math and run ahead into
+//                   the CTA's next tile.
+//   consumer warps: wait on "full", run the k-chunk on the FP64 tensor pipe (DMMA m8n8k4, the only FP64
+//                   MMA shape sm_100a has in SASS), release the stage on its "empty" mbarrier.  No
+//                   __syncthreads, no global loads and no address arithmetic in the main loop.
+// A CTA handles `tiles_per_cta` consecutive tiles of the launch's (heaviest-first) tile list, so the
+// pipeline fill and the epilogue of short-K tiles overlap with the neighbouring tiles' loads.
+// Measured on B200: with the copies issued by the MMA warps themselves and a
+// __syncthreads per stage every tile shape topped out at 70 % of the DMMA peak; TMA bulk copies
+// (cp.async.bulk) cost ~57 clk per copy per SM whatever their size, which starves the K-contiguous
+// operand format (one 128-byte row per copy); dedicated cp.async warps reach 92-95 % in the same test.
 #include "gemm.cuh"
 
 namespace dmrg {
@@ -11,14 +23,32 @@ namespace {
 constexpr int KC = 16;        // K extent of one pipeline stage
 constexpr int PK = KC + 4;    // pitch of the K-contiguous tile format [x][k]   (conflict-free LDS.64)
 
-__device__ __forceinline__ void cp_async16(void* smem, const void* gmem) {
-  unsigned s = static_cast<unsigned>(__cvta_generic_to_shared(smem));
-  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(s), "l"(gmem));
+__device__ __forceinline__ unsigned smem_u32(const void* p) { return static_cast<unsigned>(__cvta_generic_to_shared(p)); }
+
+__device__ __forceinline__ void mbar_init(unsigned long long* bar, int count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" ::"r"(smem_u32(bar)), "r"(count));
 }
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::); }
-template <int N>
-__device__ __forceinline__ void cp_async_wait() {
-  asm volatile("cp.async.wait_group %0;\n" ::"n"(N));
+__device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned parity) {
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "LAB_WAIT:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+      "@p bra LAB_DONE;\n"
+      "bra LAB_WAIT;\n"
+      "LAB_DONE:\n"
+      "}\n" ::"r"(smem_u32(bar)), "r"(parity)
+      : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(unsigned long long* bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];\n" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void cp_async16(void* smem, const void* gmem) {
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(smem_u32(smem)), "l"(gmem));
+}
+// the mbarrier receives one (pre-counted) arrival once all prior cp.async of this thread have landed
+__device__ __forceinline__ void cp_async_arrive(unsigned long long* bar) {
+  asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];\n" ::"r"(smem_u32(bar)) : "memory");
 }
 __device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double b) {
   asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
@@ -26,10 +56,17 @@ __device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double
                : "d"(a), "d"(b));
 }
 
-// Walks the flattened (segment, repeat, k-chunk) space of one output.
+constexpr int SEGW = sizeof(GSeg) / 8;   // 64-bit words per segment descriptor
+constexpr int SEGCACHE = 32;             // descriptors staged in shared memory per producer warp
+static_assert(sizeof(GSeg) % 8 == 0, "GSeg is copied as 64-bit words");
+
+// Walks the flattened (segment, repeat, k-chunk) space of one output (producer warps only; all lanes of
+// a warp walk in lockstep).  Segment descriptors are staged 32 at a time in a per-warp shared-memory
+// cache with one coalesced read, so a list of short segments costs one global latency per 32 of them.
 struct ChunkIter {
-  int seg, seg_end, rep, k0, batch;
+  int seg, seg_end, rep, k0, batch, cbase, lane;
   const GSeg* segs;
+  unsigned long long* cache;
   const double* A;
   const double* B;
   long long rsA, rsB, ams, bns;
@@ -38,18 +75,28 @@ struct ChunkIter {
   double alpha;
   __device__ __forceinline__ void load_seg() {
     if (seg < seg_end) {
-      const GSeg& s = segs[seg];
+      if (seg >= cbase + SEGCACHE) {
+        __syncwarp();
+        cbase = seg;
+        const int nw = min(SEGCACHE, seg_end - seg) * SEGW;
+        const unsigned long long* src = reinterpret_cast<const unsigned long long*>(segs + seg);
+        for (int w = lane; w < nw; w += 32) cache[w] = src[w];
+        __syncwarp();
+      }
+      const GSeg& s = *reinterpret_cast<const GSeg*>(cache + (seg - cbase) * SEGW);
       A = s.A + batch * s.bsA; B = s.B + batch * s.bsB;
       rsA = s.rsA; rsB = s.rsB; ams = s.ams; bns = s.bns; amr = s.amr; bnr = s.bnr;
       amr_inv = s.amr_inv; bnr_inv = s.bnr_inv;
       lda = s.lda; ldb = s.ldb; K = s.K; count = s.count; flags = s.flags; alpha = s.alpha;
     }
   }
-  __device__ __forceinline__ void init(const GSeg* sg, int b, int e, int bat) {
-    segs = sg; seg = b; seg_end = e; rep = 0; k0 = 0; batch = bat;
+  __device__ __forceinline__ void init(const GSeg* sg, int b, int e, int bat, unsigned long long* c, int ln) {
+    segs = sg; seg = b; seg_end = e; rep = 0; k0 = 0; batch = bat; cache = c; lane = ln;
+    cbase = b - SEGCACHE;   // forces the first fill
     load_seg();
   }
   __device__ __forceinline__ bool valid() const { return seg < seg_end; }
+  __device__ __forceinline__ bool last() const { return k0 + KC >= K && rep + 1 >= count && seg + 1 >= seg_end; }
   __device__ __forceinline__ void next() {
     k0 += KC;
     if (k0 >= K) {
@@ -59,7 +106,7 @@ struct ChunkIter {
   }
 };
 
-// element offset of logical row/col x (0-based in the whole operand) for a segmented operand
+// element offset of logical row/col x (0-based in the whole operand) for a segmented (stacked) operand
 __device__ __forceinline__ long long seg_off(int x, int nr, unsigned inv, long long stride, int& local) {
   if (nr == 0) { local = x; return 0; }
   int b = (int)__umulhi((unsigned)x, inv);
@@ -67,18 +114,18 @@ __device__ __forceinline__ long long seg_off(int x, int nr, unsigned inv, long l
   return (long long)b * stride;
 }
 
-// Copy one operand tile into shared memory.  BX = tile extent in the non-K dimension.
+// Producer: copy one operand tile of a k-chunk into shared memory, 16 bytes per cp.async, NPT threads.
+// BX = tile extent in the non-K dimension, ext = valid extent (multiple of 8), kv = valid k (8 or 16).
 //   xcontig == 0: element (x, k) at src[x*ld + k]  -> smem [x][k], pitch PK
 //   xcontig == 1: element (x, k) at src[k*ld + x]  -> smem [k][x], pitch BX + 4
-template <int BX, int NT>
-__device__ __forceinline__ void load_tile(double* sm, const double* base, int ld, int x0, int ext, int k0,
-                                          int kv, int xcontig, int nr, unsigned inv, long long stride, int tid) {
-  constexpr int ITERS = (BX * KC / 2) / NT;
-  static_assert(ITERS >= 1, "tile too small for the loader");
+template <int BX, int NPT>
+__device__ __forceinline__ void produce_tile(double* sm, const double* base, int ld, int x0, int ext, int k0, int kv,
+                                             int xcontig, int nr, unsigned inv, long long stride, int pt) {
+  constexpr int ITERS = (BX * KC / 2 + NPT - 1) / NPT;
   if (!xcontig) {
 #pragma unroll
     for (int it = 0; it < ITERS; ++it) {
-      int c = tid + it * NT;
+      int c = pt + it * NPT;
       int x = c / (KC / 2), kk = (c % (KC / 2)) * 2;
       if (x < ext && kk < kv) {
         int loc;
@@ -89,7 +136,7 @@ __device__ __forceinline__ void load_tile(double* sm, const double* base, int ld
   } else {
 #pragma unroll
     for (int it = 0; it < ITERS; ++it) {
-      int c = tid + it * NT;
+      int c = pt + it * NPT;
       int kr = c / (BX / 2), xx = (c % (BX / 2)) * 2;
       if (kr < kv && xx < ext) {
         int loc;
@@ -101,14 +148,13 @@ __device__ __forceinline__ void load_tile(double* sm, const double* base, int ld
 }
 
 // One pipeline stage of MMAs with compile-time shared-memory offsets.
-template <int BM, int BN, int FA, int FB, bool AX, bool BX>
+template <int BM, int BN, int FA, int FB, bool AX, bool BX, bool SCALE>
 __device__ __forceinline__ void compute_stage(double (&acc)[FA][FB][2], const double* sA, const double* sB,
                                               int wm0, int wn0, int lr, int lk, int kv, double alpha) {
   constexpr int SAM = AX ? 1 : PK, SAK = AX ? (BM + 4) : 1;
   constexpr int SBN = BX ? 1 : PK, SBK = BX ? (BN + 4) : 1;
   const double* pa = sA + (wm0 + lr) * SAM + lk * SAK;
   const double* pb = sB + (wn0 + lr) * SBN + lk * SBK;
-  const bool scale = alpha != 1.0;
 #pragma unroll
   for (int kk = 0; kk < KC; kk += 4) {
     if (kk < kv) {
@@ -117,7 +163,7 @@ __device__ __forceinline__ void compute_stage(double (&acc)[FA][FB][2], const do
       for (int i = 0; i < FA; ++i) af[i] = pa[(8 * i) * SAM + kk * SAK];
 #pragma unroll
       for (int j = 0; j < FB; ++j) bf[j] = pb[(8 * j) * SBN + kk * SBK];
-      if (scale) {
+      if (SCALE) {
 #pragma unroll
         for (int j = 0; j < FB; ++j) bf[j] *= alpha;
       }
@@ -129,121 +175,159 @@ __device__ __forceinline__ void compute_stage(double (&acc)[FA][FB][2], const do
   }
 }
 
-template <int BM, int BN, int WR, int WC, int STAGES, int MINB>
-__global__ void __launch_bounds__(32 * WR * WC, MINB)
-k_grouped_gemm(const GOut* __restrict__ outs, const GSeg* __restrict__ segs, const GTile* __restrict__ tiles) {
-  constexpr int NT = 32 * WR * WC;   // threads per CTA
+struct StageMeta {
+  double alpha;
+  int kv;
+  int flags;   // bit0 ta, bit1 tb, bit2 alpha != 1, bit3 last chunk of the tile
+};
+
+template <int BM, int BN, int WR, int WC, int NP, int STAGES, int MINB>
+__global__ void __launch_bounds__(32 * (WR * WC + NP), MINB)
+k_grouped_gemm(const GOut* __restrict__ outs, const GSeg* __restrict__ segs, const GTile* __restrict__ tiles,
+               int ntiles, int tiles_per_cta) {
+  constexpr int NCW = WR * WC;   // consumer warps
+  constexpr int NPT = 32 * NP;   // producer threads
   constexpr int WM = BM / WR, WN = BN / WC, FA = WM / 8, FB = WN / 8;
   constexpr int TA = BM * PK, TB = BN * PK, STAGE = TA + TB;
+  static_assert(KC * (BM + 4) <= TA && KC * (BN + 4) <= TB, "x-contiguous format must fit the stage buffer");
   extern __shared__ __align__(16) double smem[];
-  const GTile t = tiles[blockIdx.x];
-  const GOut o = outs[t.out];
+  __shared__ __align__(8) unsigned long long full_bar[STAGES], empty_bar[STAGES];
+  __shared__ StageMeta meta[STAGES];
+  __shared__ __align__(16) unsigned long long segcache[NP][SEGCACHE * SEGW];
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const int wm0 = (warp / WC) * WM, wn0 = (warp % WC) * WN;
-  const int m0 = t.m0, n0 = t.n0;
-  const int em = min(BM, o.M - m0), en = min(BN, o.N - n0);   // tile extents (multiples of 8)
-  const bool active = wm0 < em && wn0 < en;                    // warp-uniform
-
-  double acc[FA][FB][2];
-#pragma unroll
-  for (int i = 0; i < FA; ++i)
-#pragma unroll
-    for (int j = 0; j < FB; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
-
-  ChunkIter prod, cons;
-  prod.init(segs, o.seg_begin, o.seg_end, t.batch);
-  cons.init(segs, o.seg_begin, o.seg_end, t.batch);
-
-  auto issue = [&](int stage) {
-    if (prod.valid()) {
-      double* sA = smem + stage * STAGE;
-      double* sB = sA + TA;
-      const int kv = min(KC, prod.K - prod.k0);
-      const int ta = prod.flags & 1, tb = (prod.flags >> 1) & 1;
-      // op(A)(m,k): !ta -> A[m*lda+k] (K-contig) ; ta -> A[k*lda+m] (X-contig)
-      load_tile<BM, NT>(sA, prod.A + prod.rep * prod.rsA, prod.lda, m0, em, prod.k0, kv, ta, prod.amr,
-                    prod.amr_inv, prod.ams, tid);
-      // op(B)(k,n): !tb -> B[k*ldb+n] (X-contig) ; tb -> B[n*ldb+k] (K-contig)
-      load_tile<BN, NT>(sB, prod.B + prod.rep * prod.rsB, prod.ldb, n0, en, prod.k0, kv, !tb, prod.bnr,
-                    prod.bnr_inv, prod.bns, tid);
-      prod.next();
-    }
-    cp_async_commit();
-  };
-
-#pragma unroll
-  for (int s = 0; s < STAGES - 1; ++s) issue(s);
-
+  if (tid == 0) {
+    // full: one counted cp.async arrival per producer thread + the explicit arrival that publishes meta
+    for (int s = 0; s < STAGES; ++s) { mbar_init(&full_bar[s], NPT + 1); mbar_init(&empty_bar[s], NCW); }
+    asm volatile("fence.mbarrier_init.release.cluster;\n" ::);
+  }
+  __syncthreads();
+  const int t_begin = blockIdx.x * tiles_per_cta, t_end = min(ntiles, t_begin + tiles_per_cta);
   int stage = 0;
-  const int lr = lane >> 2, lk = lane & 3;
-  while (cons.valid()) {
-    cp_async_wait<STAGES - 2>();
-    __syncthreads();
-    issue((stage + STAGES - 1) % STAGES);
-    if (active) {
-      const double* sA = smem + stage * STAGE;
-      const double* sB = sA + TA;
-      const int kv = min(KC, cons.K - cons.k0);
-      const int ta = cons.flags & 1, tb = (cons.flags >> 1) & 1;
-      if (!ta) {
-        if (tb) compute_stage<BM, BN, FA, FB, false, false>(acc, sA, sB, wm0, wn0, lr, lk, kv, cons.alpha);
-        else compute_stage<BM, BN, FA, FB, false, true>(acc, sA, sB, wm0, wn0, lr, lk, kv, cons.alpha);
-      } else {
-        if (tb) compute_stage<BM, BN, FA, FB, true, false>(acc, sA, sB, wm0, wn0, lr, lk, kv, cons.alpha);
-        else compute_stage<BM, BN, FA, FB, true, true>(acc, sA, sB, wm0, wn0, lr, lk, kv, cons.alpha);
+  unsigned phase = 0;
+
+  if (warp >= NCW) {
+    // ------------------------------------------------ producers ------------------------------------------------
+    const int pt = tid - 32 * NCW;
+    for (int ti = t_begin; ti < t_end; ++ti) {
+      const GTile t = tiles[ti];
+      const GOut o = outs[t.out];
+      const int em = min(BM, o.M - t.m0), en = min(BN, o.N - t.n0);
+      ChunkIter it;
+      it.init(segs, o.seg_begin, o.seg_end, t.batch, segcache[warp - NCW], lane);
+      while (it.valid()) {
+        mbar_wait(&empty_bar[stage], phase ^ 1);
+        double* sA = smem + stage * STAGE;
+        double* sB = sA + TA;
+        const int kv = min(KC, it.K - it.k0);
+        const int ta = it.flags & 1, tb = (it.flags >> 1) & 1;
+        if (pt == 0) {
+          meta[stage] = StageMeta{it.alpha, kv, (it.flags & 3) | (it.alpha != 1.0 ? 4 : 0) | (it.last() ? 8 : 0)};
+          mbar_arrive(&full_bar[stage]);
+        }
+        // op(A)(m,k): !ta -> A[m*lda+k] (K-contig) ; ta -> A[k*lda+m] (X-contig)
+        produce_tile<BM, NPT>(sA, it.A + it.rep * it.rsA, it.lda, t.m0, em, it.k0, kv, ta, it.amr, it.amr_inv, it.ams, pt);
+        // op(B)(k,n): !tb -> B[k*ldb+n] (X-contig) ; tb -> B[n*ldb+k] (K-contig)
+        produce_tile<BN, NPT>(sB, it.B + it.rep * it.rsB, it.ldb, t.n0, en, it.k0, kv, !tb, it.bnr, it.bnr_inv, it.bns, pt);
+        cp_async_arrive(&full_bar[stage]);
+        it.next();
+        if (++stage == STAGES) { stage = 0; phase ^= 1; }
       }
     }
-    cons.next();
-    stage = (stage + 1) % STAGES;
+    asm volatile("cp.async.wait_all;\n" ::);
+    return;
   }
-  cp_async_wait<0>();
 
-  if (!active) return;
-  double* C = o.C + (long long)t.batch * o.bsC;
+  // ---------------------------------------------------- consumers ----------------------------------------------------
+  const int wm0 = (warp / WC) * WM, wn0 = (warp % WC) * WN;
+  const int lr = lane >> 2, lk = lane & 3;
+  for (int ti = t_begin; ti < t_end; ++ti) {
+    const GTile t = tiles[ti];
+    const GOut o = outs[t.out];
+    const int m0 = t.m0, n0 = t.n0;
+    const int em = min(BM, o.M - m0), en = min(BN, o.N - n0);   // tile extents (multiples of 8)
+    const bool active = wm0 < em && wn0 < en;                    // warp-uniform
+    double acc[FA][FB][2];
 #pragma unroll
-  for (int i = 0; i < FA; ++i) {
-    const int rl = wm0 + 8 * i;
-    if (rl < em) {
+    for (int i = 0; i < FA; ++i)
 #pragma unroll
-      for (int j = 0; j < FB; ++j) {
-        const int cl = wn0 + 8 * j;
-        if (cl < en) {
-          double2* p = reinterpret_cast<double2*>(C + (long long)(m0 + rl + lr) * o.ldc + n0 + cl + 2 * lk);
-          double2 v = make_double2(acc[i][j][0], acc[i][j][1]);
-          if (o.accumulate) {
-            double2 old = *p;
-            v.x += old.x; v.y += old.y;
+      for (int j = 0; j < FB; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
+
+    bool more = o.seg_begin < o.seg_end;
+    while (more) {
+      mbar_wait(&full_bar[stage], phase);
+      const StageMeta mt = meta[stage];
+      if (active) {
+        const double* sA = smem + stage * STAGE;
+        const double* sB = sA + TA;
+        switch (mt.flags & 7) {
+          case 0: compute_stage<BM, BN, FA, FB, false, true, false>(acc, sA, sB, wm0, wn0, lr, lk, mt.kv, 1.0); break;
+          case 1: compute_stage<BM, BN, FA, FB, true, true, false>(acc, sA, sB, wm0, wn0, lr, lk, mt.kv, 1.0); break;
+          case 2: compute_stage<BM, BN, FA, FB, false, false, false>(acc, sA, sB, wm0, wn0, lr, lk, mt.kv, 1.0); break;
+          case 3: compute_stage<BM, BN, FA, FB, true, false, false>(acc, sA, sB, wm0, wn0, lr, lk, mt.kv, 1.0); break;
+          case 4: compute_stage<BM, BN, FA, FB, false, true, true>(acc, sA, sB, wm0, wn0, lr, lk, mt.kv, mt.alpha); break;
+          case 5: compute_stage<BM, BN, FA, FB, true, true, true>(acc, sA, sB, wm0, wn0, lr, lk, mt.kv, mt.alpha); break;
+          case 6: compute_stage<BM, BN, FA, FB, false, false, true>(acc, sA, sB, wm0, wn0, lr, lk, mt.kv, mt.alpha); break;
+          default: compute_stage<BM, BN, FA, FB, true, false, true>(acc, sA, sB, wm0, wn0, lr, lk, mt.kv, mt.alpha); break;
+        }
+      }
+      __syncwarp();
+      if (lane == 0) mbar_arrive(&empty_bar[stage]);
+      more = !(mt.flags & 8);
+      if (++stage == STAGES) { stage = 0; phase ^= 1; }
+    }
+
+    if (!active) continue;
+    // epilogue: one 8-row fragment strip (FB double2 per thread) at a time; for accumulating outputs all
+    // loads of a strip are issued before its adds and stores, so the read latency is paid once per strip
+    double* C = o.C + (long long)t.batch * o.bsC + (long long)(m0 + wm0 + lr) * o.ldc + n0 + wn0 + 2 * lk;
+#pragma unroll
+    for (int i = 0; i < FA; ++i) {
+      if (wm0 + 8 * i < em) {
+        double2* row = reinterpret_cast<double2*>(C + (long long)(8 * i) * o.ldc);
+        double2 old[FB];
+        if (o.accumulate) {
+#pragma unroll
+          for (int j = 0; j < FB; ++j)
+            if (wn0 + 8 * j < en) old[j] = row[4 * j];
+        }
+#pragma unroll
+        for (int j = 0; j < FB; ++j) {
+          if (wn0 + 8 * j < en) {
+            double2 v = make_double2(acc[i][j][0], acc[i][j][1]);
+            if (o.accumulate) { v.x += old[j].x; v.y += old[j].y; }
+            row[4 * j] = v;
           }
-          *p = v;
         }
       }
     }
   }
 }
 
-template <int BM, int BN, int WR, int WC, int STAGES, int MINB>
+template <int BM, int BN, int WR, int WC, int NP, int STAGES, int MINB>
 struct Cfg {
   static constexpr int smem = STAGES * (BM + BN) * PK * 8;
+  static constexpr int threads = 32 * (WR * WC + NP);
+  static constexpr int minb = MINB;
   static cudaError_t init() {
-    return cudaFuncSetAttribute(k_grouped_gemm<BM, BN, WR, WC, STAGES, MINB>,
+    return cudaFuncSetAttribute(k_grouped_gemm<BM, BN, WR, WC, NP, STAGES, MINB>,
                                 cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
   }
-  static cudaError_t launch(const GOut* o, const GSeg* s, const GTile* t, int n, cudaStream_t st) {
-    k_grouped_gemm<BM, BN, WR, WC, STAGES, MINB><<<n, 32 * WR * WC, smem, st>>>(o, s, t);
+  static cudaError_t launch(const GOut* o, const GSeg* s, const GTile* t, int n, int per, cudaStream_t st) {
+    k_grouped_gemm<BM, BN, WR, WC, NP, STAGES, MINB><<<(n + per - 1) / per, threads, smem, st>>>(o, s, t, n, per);
     return cudaGetLastError();
   }
 };
 
-//                 BM   BN  WR WC ST MINB
-using S32x32   = Cfg<32, 32, 2, 4, 3, 4>;
-using S32x64   = Cfg<32, 64, 2, 4, 3, 4>;
-using S32x128  = Cfg<32, 128, 1, 8, 3, 3>;
-using S64x32   = Cfg<64, 32, 4, 2, 3, 4>;
-using S64x64   = Cfg<64, 64, 2, 4, 3, 3>;
-using S64x128  = Cfg<64, 128, 2, 4, 3, 2>;
-using S128x32  = Cfg<128, 32, 8, 1, 3, 3>;
-using S128x64  = Cfg<128, 64, 4, 2, 3, 2>;
-using S128x128 = Cfg<128, 128, 4, 4, 4, 1>;
+//                 BM   BN  WR WC NP ST MINB     warp tile
+using S32x32   = Cfg<32, 32, 1, 1, 1, 6, 4>;   // 32x32
+using S32x64   = Cfg<32, 64, 1, 2, 1, 6, 3>;   // 32x32
+using S32x128  = Cfg<32, 128, 1, 4, 2, 4, 2>;  // 32x32
+using S64x32   = Cfg<64, 32, 2, 1, 1, 6, 3>;   // 32x32
+using S64x64   = Cfg<64, 64, 2, 2, 2, 4, 2>;   // 32x32
+using S64x128  = Cfg<64, 128, 1, 4, 2, 3, 2>;  // 64x32
+using S128x32  = Cfg<128, 32, 4, 1, 2, 4, 2>;  // 32x32
+using S128x64  = Cfg<128, 64, 2, 2, 2, 3, 2>;  // 64x32
+using S128x128 = Cfg<128, 128, 2, 4, 4, 4, 1>; // 64x32
 
 }  // namespace
 
@@ -260,18 +344,34 @@ cudaError_t grouped_gemm_init() {
   return S128x128::init();
 }
 
-cudaError_t launch_grouped_gemm(int shape, const GOut* o, const GSeg* s, const GTile* t, int n, cudaStream_t st) {
-  if (n <= 0) return cudaSuccess;
+int gemm_shape_ctas_per_sm(int shape) {
   switch (shape) {
-    case 0: return S32x32::launch(o, s, t, n, st);
-    case 1: return S32x64::launch(o, s, t, n, st);
-    case 2: return S32x128::launch(o, s, t, n, st);
-    case 3: return S64x32::launch(o, s, t, n, st);
-    case 4: return S64x64::launch(o, s, t, n, st);
-    case 5: return S64x128::launch(o, s, t, n, st);
-    case 6: return S128x32::launch(o, s, t, n, st);
-    case 7: return S128x64::launch(o, s, t, n, st);
-    case 8: return S128x128::launch(o, s, t, n, st);
+    case 0: return S32x32::minb;
+    case 1: return S32x64::minb;
+    case 2: return S32x128::minb;
+    case 3: return S64x32::minb;
+    case 4: return S64x64::minb;
+    case 5: return S64x128::minb;
+    case 6: return S128x32::minb;
+    case 7: return S128x64::minb;
+    default: return S128x128::minb;
+  }
+}
+
+cudaError_t launch_grouped_gemm(int shape, const GOut* o, const GSeg* s, const GTile* t, int n, int tiles_per_cta,
+                                cudaStream_t st) {
+  if (n <= 0) return cudaSuccess;
+  const int per = tiles_per_cta < 1 ? 1 : tiles_per_cta;
+  switch (shape) {
+    case 0: return S32x32::launch(o, s, t, n, per, st);
+    case 1: return S32x64::launch(o, s, t, n, per, st);
+    case 2: return S32x128::launch(o, s, t, n, per, st);
+    case 3: return S64x32::launch(o, s, t, n, per, st);
+    case 4: return S64x64::launch(o, s, t, n, per, st);
+    case 5: return S64x128::launch(o, s, t, n, per, st);
+    case 6: return S128x32::launch(o, s, t, n, per, st);
+    case 7: return S128x64::launch(o, s, t, n, per, st);
+    case 8: return S128x128::launch(o, s, t, n, per, st);
   }
   return cudaErrorInvalidValue;
 }

@@ -1,4 +1,5 @@
-// Grouped, batched, segment-accumulating FP64 GEMM on the DMMA pipe (sm_100a).
+// Grouped, batched, segment-accumulating FP64 GEMM on the DMMA pipe (sm_100a), operands staged by TMA
+// bulk copies from a producer warp (gemm.cu).
 //
 // One launch executes a list of output tiles of ONE tile shape.  Each output matrix C (M x N) is
 //     C (+)= sum_{seg in segs(C)} sum_{r < seg.count} alpha_seg * op(A_seg[r]) * op(B_seg[r])
@@ -53,9 +54,11 @@ constexpr int GEMM_DIMS[3] = {32, 64, 128};
 inline int gemm_shape_rows(int s) { return GEMM_DIMS[s / 3]; }
 inline int gemm_shape_cols(int s) { return GEMM_DIMS[s % 3]; }
 
-// Launch `ntiles` tiles of shape `shape` (device arrays).  Returns the cudaError of the launch.
+// Launch `ntiles` tiles of shape `shape` (device arrays); every CTA takes `tiles_per_cta` consecutive
+// tiles of the list.  Returns the cudaError of the launch.
 cudaError_t launch_grouped_gemm(int shape, const GOut* d_outs, const GSeg* d_segs, const GTile* d_tiles,
-                                int ntiles, cudaStream_t stream);
+                                int ntiles, int tiles_per_cta, cudaStream_t stream);
+int gemm_shape_ctas_per_sm(int shape);   // resident CTAs per SM the shape's kernel is built for
 cudaError_t grouped_gemm_init();
 
 }  // namespace dmrg

@@ -27,6 +27,15 @@ Exec::~Exec() {
 }
 
 namespace {
+// Tiles per CTA: long lists of short tiles are batched so that the producer warp's prefetch runs across
+// tile boundaries; keep >= 16 CTAs per resident slot for load balance.
+int tiles_per_cta(int shape, int ntiles) {
+  const int slots = 148 * gemm_shape_ctas_per_sm(shape);
+  return std::max(1, std::min(8, ntiles / (slots * 16)));
+}
+cudaError_t launch_shape(const Phase& ph, int s, cudaStream_t st) {
+  return launch_grouped_gemm(s, ph.outs.p, ph.segs.p, ph.tiles[s].p, ph.ntiles[s], tiles_per_cta(s, ph.ntiles[s]), st);
+}
 struct Launch { const Phase* ph; int shape; double work; };
 void collect(const Phase& ph, std::vector<Launch>& v) {
   for (int s = GEMM_NSHAPES - 1; s >= 0; --s)
@@ -44,7 +53,7 @@ void Plan::run(cudaStream_t st, int64_t* launch_counter, Exec* ex) const {
     if (launch_counter) *launch_counter += (int64_t)ls.size();
     if (!ex || ls.size() == 1) {
       for (auto& l : ls)
-        DMRG_CUDA(launch_grouped_gemm(l.shape, l.ph->outs.p, l.ph->segs.p, l.ph->tiles[l.shape].p, l.ph->ntiles[l.shape], st));
+        DMRG_CUDA(launch_shape(*l.ph, l.shape, st));
     } else {
       std::stable_sort(ls.begin(), ls.end(), [](const Launch& a, const Launch& b) { return a.work > b.work; });
       DMRG_CUDA(cudaEventRecord(ex->fork, st));
@@ -52,8 +61,7 @@ void Plan::run(cudaStream_t st, int64_t* launch_counter, Exec* ex) const {
       for (int i = 0; i < nw; ++i) DMRG_CUDA(cudaStreamWaitEvent(ex->w[i], ex->fork, 0));
       for (size_t i = 0; i < ls.size(); ++i) {
         const Launch& l = ls[i];
-        DMRG_CUDA(launch_grouped_gemm(l.shape, l.ph->outs.p, l.ph->segs.p, l.ph->tiles[l.shape].p, l.ph->ntiles[l.shape],
-                                      ex->w[i % nw]));
+        DMRG_CUDA(launch_shape(*l.ph, l.shape, ex->w[i % nw]));
       }
       for (int i = 0; i < nw; ++i) {
         DMRG_CUDA(cudaEventRecord(ex->join[i], ex->w[i]));
@@ -83,7 +91,7 @@ void Plan::run_profiled(cudaStream_t st, std::vector<LaunchRecord>* out) const {
       const Phase& ph = p == 0 ? chunks[c].p1 : chunks[c].p2;
       for (int s = GEMM_NSHAPES - 1; s >= 0; --s) {
         if (ph.ntiles[s] <= 0) continue;
-        DMRG_CUDA(launch_grouped_gemm(s, ph.outs.p, ph.segs.p, ph.tiles[s].p, ph.ntiles[s], st));
+        DMRG_CUDA(launch_shape(ph, s, st));
         mark();
         out->push_back(LaunchRecord{(int)c, p + 1, s, ph.ntiles[s], ph.shape_flops[s], 0.f});
       }
@@ -247,28 +255,28 @@ void Planner::finish(Plan* plan, cudaStream_t st) {
   struct HRed { RedDesc d; long long p_off; };
   std::vector<std::vector<HRed>> reds(chunks_.size());
   long long scratch_max = 0;
-  auto tile_area = [](int M, int N, double* maxarea) {
-    std::vector<std::pair<int, int>> rs, cs;
-    split_dim(M, rs); split_dim(N, cs);
-    double a = 0, mx = 0;
-    for (auto& r : rs) for (auto& c : cs) {
-      double t = (double)GEMM_DIMS[r.second] * GEMM_DIMS[c.second];
-      a += t; mx = std::max(mx, t);
-    }
-    *maxarea = mx;
-    return a;
-  };
   for (size_t ci = 0; ci < chunks_.size(); ++ci) {
     std::vector<HOut>& hv = chunks_[ci].p2;
+    // cost model of one tile: k-chunks x max(tile area, 8192) -- a narrow tile is latency-bound and takes
+    // about as long per k-chunk as a 64x128 one.  Outputs are cut so that no tile part exceeds 1/16 of
+    // the per-SM share of the chunk.
     double total = 0;
     std::vector<double> ks(hv.size()), mxa(hv.size());
     for (size_t i = 0; i < hv.size(); ++i) {
       double k = 0;
       for (auto& hs : hv[i].segs) k += (double)hs.s.K * hs.s.count;
       ks[i] = k;
-      total += k * tile_area(hv[i].o.M, hv[i].o.N, &mxa[i]) * hv[i].batch;
+      std::vector<std::pair<int, int>> rs, cs;
+      split_dim(hv[i].o.M, rs); split_dim(hv[i].o.N, cs);
+      double mx = 0;
+      for (auto& r : rs) for (auto& c : cs) {
+        double t = std::max(8192.0, (double)GEMM_DIMS[r.second] * GEMM_DIMS[c.second]);
+        total += k * t * hv[i].batch;
+        mx = std::max(mx, t);
+      }
+      mxa[i] = mx;
     }
-    const double wstar = total / (148.0 * 6.0);
+    const double wstar = total / (148.0 * 16.0);
     std::vector<HOut> ex;
     long long sc_used = 0;
     for (size_t i = 0; i < hv.size(); ++i) {
@@ -276,7 +284,7 @@ void Planner::finish(Plan* plan, cudaStream_t st) {
       long long units = 0;
       for (auto& hs : h.segs) units += hs.s.count;
       int ns = wstar > 0 ? (int)std::ceil(ks[i] * mxa[i] / wstar) : 1;
-      ns = (int)std::min<long long>(std::min(ns, 16), units);
+      ns = (int)std::min<long long>(std::min(ns, 32), units);
       if (ns <= 1) { ex.push_back(std::move(h)); continue; }
       const long long mn = (long long)h.o.M * h.o.N;
       HRed rd{};
