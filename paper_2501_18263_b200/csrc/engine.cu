@@ -268,14 +268,16 @@ std::unique_ptr<BlockSide> vacuum_block(dmrg_ctx* ctx, bool is_left, cudaStream_
   return B;
 }
 
-// Workspace cap for the O_L.psi intermediates: the caller's, else a third of the free device memory
-// (1..64 GB).  Fewer, larger chunks mean fewer under-filled launch tails per apply.
+// Workspace cap for the O_L.psi intermediates: the caller's, else 40 % of the device memory this context
+// has not allocated itself (1..64 GB).  Fewer, larger chunks mean fewer under-filled launch tails per
+// apply.  (cudaMemGetInfo is no guide here: the caller's allocator may cache freed blocks.)
 static uint64_t workspace_cap(const dmrg_ctx* ctx) {
   if (ctx->cfg.workspace_bytes) return ctx->cfg.workspace_bytes;
   size_t fr = 0, tot = 0;
   if (cudaMemGetInfo(&fr, &tot) != cudaSuccess) return 16ull << 30;
-  uint64_t cap = fr / 3;
-  return std::min<uint64_t>(std::max<uint64_t>(cap, 1ull << 30), 64ull << 30);
+  const uint64_t mine = ctx->al.live_bytes;
+  const uint64_t rest = tot > mine ? tot - mine : 0;
+  return std::min<uint64_t>(std::max<uint64_t>(rest / 5 * 2, 1ull << 30), 64ull << 30);
 }
 
 static inline uint64_t pack_key(int a, int b, int c, int d, int e, int f) {

@@ -175,11 +175,17 @@ __device__ __forceinline__ void compute_stage(double (&acc)[FA][FB][2], const do
   }
 }
 
+// What the producers tell the consumers about a stage.  The first chunk of a tile also carries the
+// tile itself, so the consumer warps never read a descriptor from global memory.
 struct StageMeta {
   double alpha;
+  double* C;      // first chunk of a tile: element (m0, n0) of the output (batch applied)
   int kv;
-  int flags;   // bit0 ta, bit1 tb, bit2 alpha != 1, bit3 last chunk of the tile
+  int flags;      // bit0 ta, bit1 tb, bit2 alpha != 1, bit3 last chunk of the tile, bit4 first chunk of the
+                  // tile, bit5 last chunk of the CTA, bit6 output accumulates
+  int ldc, em, en, pad_;
 };
+enum : int { F_LAST = 8, F_FIRST = 16, F_FINAL = 32, F_ACC = 64 };
 
 template <int BM, int BN, int WR, int WC, int NP, int STAGES, int MINB>
 __global__ void __launch_bounds__(32 * (WR * WC + NP), MINB)
@@ -192,7 +198,7 @@ k_grouped_gemm(const GOut* __restrict__ outs, const GSeg* __restrict__ segs, con
   static_assert(KC * (BM + 4) <= TA && KC * (BN + 4) <= TB, "x-contiguous format must fit the stage buffer");
   extern __shared__ __align__(16) double smem[];
   __shared__ __align__(8) unsigned long long full_bar[STAGES], empty_bar[STAGES];
-  __shared__ StageMeta meta[STAGES];
+  __shared__ __align__(16) StageMeta meta[STAGES];
   __shared__ __align__(16) unsigned long long segcache[NP][SEGCACHE * SEGW];
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   if (tid == 0) {
@@ -201,19 +207,23 @@ k_grouped_gemm(const GOut* __restrict__ outs, const GSeg* __restrict__ segs, con
     asm volatile("fence.mbarrier_init.release.cluster;\n" ::);
   }
   __syncthreads();
-  const int t_begin = blockIdx.x * tiles_per_cta, t_end = min(ntiles, t_begin + tiles_per_cta);
   int stage = 0;
   unsigned phase = 0;
 
   if (warp >= NCW) {
     // ------------------------------------------------ producers ------------------------------------------------
+    // (every tile of the list has at least one k-chunk: the planner emits no tiles for empty outputs)
     const int pt = tid - 32 * NCW;
+    const int t_begin = blockIdx.x * tiles_per_cta, t_end = min(ntiles, t_begin + tiles_per_cta);
+    GTile tn = tiles[t_begin];
     for (int ti = t_begin; ti < t_end; ++ti) {
-      const GTile t = tiles[ti];
+      const GTile t = tn;
+      if (ti + 1 < t_end) tn = tiles[ti + 1];   // in flight while this tile streams
       const GOut o = outs[t.out];
       const int em = min(BM, o.M - t.m0), en = min(BN, o.N - t.n0);
       ChunkIter it;
       it.init(segs, o.seg_begin, o.seg_end, t.batch, segcache[warp - NCW], lane);
+      bool first = true;
       while (it.valid()) {
         mbar_wait(&empty_bar[stage], phase ^ 1);
         double* sA = smem + stage * STAGE;
@@ -221,9 +231,18 @@ k_grouped_gemm(const GOut* __restrict__ outs, const GSeg* __restrict__ segs, con
         const int kv = min(KC, it.K - it.k0);
         const int ta = it.flags & 1, tb = (it.flags >> 1) & 1;
         if (pt == 0) {
-          meta[stage] = StageMeta{it.alpha, kv, (it.flags & 3) | (it.alpha != 1.0 ? 4 : 0) | (it.last() ? 8 : 0)};
+          const bool last = it.last();
+          StageMeta m;
+          m.alpha = it.alpha;
+          m.C = o.C + (long long)t.batch * o.bsC + (long long)t.m0 * o.ldc + t.n0;
+          m.kv = kv;
+          m.flags = (it.flags & 3) | (it.alpha != 1.0 ? 4 : 0) | (last ? F_LAST : 0) | (first ? F_FIRST : 0) |
+                    (last && ti + 1 == t_end ? F_FINAL : 0) | (o.accumulate ? F_ACC : 0);
+          m.ldc = o.ldc; m.em = em; m.en = en; m.pad_ = 0;
+          meta[stage] = m;
           mbar_arrive(&full_bar[stage]);
         }
+        first = false;
         // op(A)(m,k): !ta -> A[m*lda+k] (K-contig) ; ta -> A[k*lda+m] (X-contig)
         produce_tile<BM, NPT>(sA, it.A + it.rep * it.rsA, it.lda, t.m0, em, it.k0, kv, ta, it.amr, it.amr_inv, it.ams, pt);
         // op(B)(k,n): !tb -> B[k*ldb+n] (X-contig) ; tb -> B[n*ldb+k] (K-contig)
@@ -238,68 +257,69 @@ k_grouped_gemm(const GOut* __restrict__ outs, const GSeg* __restrict__ segs, con
   }
 
   // ---------------------------------------------------- consumers ----------------------------------------------------
+  // One stream of stages; tile boundaries are flags in the stage meta.
   const int wm0 = (warp / WC) * WM, wn0 = (warp % WC) * WN;
   const int lr = lane >> 2, lk = lane & 3;
-  for (int ti = t_begin; ti < t_end; ++ti) {
-    const GTile t = tiles[ti];
-    const GOut o = outs[t.out];
-    const int m0 = t.m0, n0 = t.n0;
-    const int em = min(BM, o.M - m0), en = min(BN, o.N - n0);   // tile extents (multiples of 8)
-    const bool active = wm0 < em && wn0 < en;                    // warp-uniform
-    double acc[FA][FB][2];
+  double acc[FA][FB][2];
+  double* C = nullptr;
+  int ldc = 0, em = 0, en = 0, accum = 0;
+  bool active = false;
+  while (true) {
+    mbar_wait(&full_bar[stage], phase);
+    const StageMeta mt = meta[stage];
+    if (mt.flags & F_FIRST) {
+      C = mt.C; ldc = mt.ldc; em = mt.em; en = mt.en; accum = mt.flags & F_ACC;
+      active = wm0 < em && wn0 < en;   // warp-uniform
 #pragma unroll
-    for (int i = 0; i < FA; ++i)
+      for (int i = 0; i < FA; ++i)
 #pragma unroll
-      for (int j = 0; j < FB; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
-
-    bool more = o.seg_begin < o.seg_end;
-    while (more) {
-      mbar_wait(&full_bar[stage], phase);
-      const StageMeta mt = meta[stage];
-      if (active) {
-        const double* sA = smem + stage * STAGE;
-        const double* sB = sA + TA;
-        switch (mt.flags & 7) {
-          case 0: compute_stage<BM, BN, FA, FB, false, true, false>(acc, sA, sB, wm0, wn0, lr, lk, mt.kv, 1.0); break;
-          case 1: compute_stage<BM, BN, FA, FB, true, true, false>(acc, sA, sB, wm0, wn0, lr, lk, mt.kv, 1.0); break;
-          case 2: compute_stage<BM, BN, FA, FB, false, false, false>(acc, sA, sB, wm0, wn0, lr, lk, mt.kv, 1.0); break;
-          case 3: compute_stage<BM, BN, FA, FB, true, false, false>(acc, sA, sB, wm0, wn0, lr, lk, mt.kv, 1.0); break;
-          case 4: compute_stage<BM, BN, FA, FB, false, true, true>(acc, sA, sB, wm0, wn0, lr, lk, mt.kv, mt.alpha); break;
-          case 5: compute_stage<BM, BN, FA, FB, true, true, true>(acc, sA, sB, wm0, wn0, lr, lk, mt.kv, mt.alpha); break;
-          case 6: compute_stage<BM, BN, FA, FB, false, false, true>(acc, sA, sB, wm0, wn0, lr, lk, mt.kv, mt.alpha); break;
-          default: compute_stage<BM, BN, FA, FB, true, false, true>(acc, sA, sB, wm0, wn0, lr, lk, mt.kv, mt.alpha); break;
-        }
-      }
-      __syncwarp();
-      if (lane == 0) mbar_arrive(&empty_bar[stage]);
-      more = !(mt.flags & 8);
-      if (++stage == STAGES) { stage = 0; phase ^= 1; }
+        for (int j = 0; j < FB; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
     }
+    if (active) {
+      const double* sA = smem + stage * STAGE;
+      const double* sB = sA + TA;
+      switch (mt.flags & 7) {
+        case 0: compute_stage<BM, BN, FA, FB, false, true, false>(acc, sA, sB, wm0, wn0, lr, lk, mt.kv, 1.0); break;
+        case 1: compute_stage<BM, BN, FA, FB, true, true, false>(acc, sA, sB, wm0, wn0, lr, lk, mt.kv, 1.0); break;
+        case 2: compute_stage<BM, BN, FA, FB, false, false, false>(acc, sA, sB, wm0, wn0, lr, lk, mt.kv, 1.0); break;
+        case 3: compute_stage<BM, BN, FA, FB, true, false, false>(acc, sA, sB, wm0, wn0, lr, lk, mt.kv, 1.0); break;
+        case 4: compute_stage<BM, BN, FA, FB, false, true, true>(acc, sA, sB, wm0, wn0, lr, lk, mt.kv, mt.alpha); break;
+        case 5: compute_stage<BM, BN, FA, FB, true, true, true>(acc, sA, sB, wm0, wn0, lr, lk, mt.kv, mt.alpha); break;
+        case 6: compute_stage<BM, BN, FA, FB, false, false, true>(acc, sA, sB, wm0, wn0, lr, lk, mt.kv, mt.alpha); break;
+        default: compute_stage<BM, BN, FA, FB, true, false, true>(acc, sA, sB, wm0, wn0, lr, lk, mt.kv, mt.alpha); break;
+      }
+    }
+    __syncwarp();
+    if (lane == 0) mbar_arrive(&empty_bar[stage]);
+    if (++stage == STAGES) { stage = 0; phase ^= 1; }
+    if (!(mt.flags & F_LAST)) continue;
 
-    if (!active) continue;
-    // epilogue: one 8-row fragment strip (FB double2 per thread) at a time; for accumulating outputs all
-    // loads of a strip are issued before its adds and stores, so the read latency is paid once per strip
-    double* C = o.C + (long long)t.batch * o.bsC + (long long)(m0 + wm0 + lr) * o.ldc + n0 + wn0 + 2 * lk;
+    if (active) {
+      // epilogue: one 8-row fragment strip (FB double2 per thread) at a time; for accumulating outputs all
+      // loads of a strip are issued before its adds and stores, so the read latency is paid once per strip
+      double* Cw = C + (long long)(wm0 + lr) * ldc + wn0 + 2 * lk;
 #pragma unroll
-    for (int i = 0; i < FA; ++i) {
-      if (wm0 + 8 * i < em) {
-        double2* row = reinterpret_cast<double2*>(C + (long long)(8 * i) * o.ldc);
-        double2 old[FB];
-        if (o.accumulate) {
+      for (int i = 0; i < FA; ++i) {
+        if (wm0 + 8 * i < em) {
+          double2* row = reinterpret_cast<double2*>(Cw + (long long)(8 * i) * ldc);
+          double2 old[FB];
+          if (accum) {
 #pragma unroll
-          for (int j = 0; j < FB; ++j)
-            if (wn0 + 8 * j < en) old[j] = row[4 * j];
-        }
+            for (int j = 0; j < FB; ++j)
+              if (wn0 + 8 * j < en) old[j] = row[4 * j];
+          }
 #pragma unroll
-        for (int j = 0; j < FB; ++j) {
-          if (wn0 + 8 * j < en) {
-            double2 v = make_double2(acc[i][j][0], acc[i][j][1]);
-            if (o.accumulate) { v.x += old[j].x; v.y += old[j].y; }
-            row[4 * j] = v;
+          for (int j = 0; j < FB; ++j) {
+            if (wn0 + 8 * j < en) {
+              double2 v = make_double2(acc[i][j][0], acc[i][j][1]);
+              if (accum) { v.x += old[j].x; v.y += old[j].y; }
+              row[4 * j] = v;
+            }
           }
         }
       }
     }
+    if (mt.flags & F_FINAL) break;
   }
 }
 

@@ -355,6 +355,7 @@ void Planner::finish(Plan* plan, cudaStream_t st) {
       }
       o.seg_end = (int)segs.size();
       outs.push_back(o);
+      if (o.seg_begin == o.seg_end) continue;   // nothing to add: the kernel needs >= 1 k-chunk per tile
       std::vector<std::pair<int, int>> rs, cs;
       split_dim(o.M, rs);
       split_dim(o.N, cs);
