@@ -234,3 +234,202 @@ def make_config(cfg: int, D: int | None = None, k: int | None = None):
     kk = L // 2 if k is None else k
     mps = make_mps(L, c["n_up"], c["n_dn"], c["D"] if D is None else D, kk, c["seed"])
     return T, V, mps
+
+
+# =================================================================================================
+# SU(2)-adapted inputs (BASELINE.json configs[3] second half and configs[4]).
+# A bond sector is labelled q = (N, 2S): N electrons and total spin S in sites 1..b.  The site carries
+# three multiplets m = 0, 1, 2 = (N=0,S=0), (N=1,S=1/2), (N=2,S=0).  A reduced site
+# tensor block is keyed (q_in, m, q_out) with q_out = (N_in + n(m), 2S_in + {0 | +-1}); shapes
+# (d_in, d_out), counted in multiplets.  Still no method arithmetic here: only sizes and random isometries.
+# =================================================================================================
+SITE_MULT = ((0, 0), (1, 1), (2, 0))   # (N, 2S) of the site multiplets m = 0, 1, 2
+
+
+def su2_couplings(q, m):
+    """Bond labels reachable from q = (N, 2S) by adding site multiplet m."""
+    n, s2 = SITE_MULT[m]
+    if s2 == 0:
+        return [(q[0] + n, q[1])]
+    out = [(q[0] + n, q[1] + 1)]
+    if q[1] >= 1:
+        out.append((q[0] + n, q[1] - 1))
+    return out
+
+
+def _mult_count(b, N, S2):
+    """Number of (N, S) multiplets of b orbitals: #(N, Sz=S) - #(N, Sz=S+1), #(N,Sz) = C(b,na) C(b,nb)."""
+    def cnt(sz2):
+        if (N + sz2) % 2:
+            return 0
+        na, nb = (N + sz2) // 2, (N - sz2) // 2
+        return _binom(b, na) * _binom(b, nb)
+    return cnt(S2) - cnt(S2 + 2)
+
+
+def su2_bond_sectors(L: int, N_tot: int, S2_tot: int, D: int):
+    """Multiplet counts d_b(N, 2S) for every bond: weight m_b(N,S) * m_{L-b}(N_tot-N, S) (target S_tot = 0:
+    the right part carries the same S; for S_tot != 0 the sum over the allowed right spins), cap = min of
+    the two factors, water-filling to D multiplets, largest-remainder rounding, clipping passes."""
+    secs = []
+    for b in range(L + 1):
+        cand = {}
+        for N in range(0, min(2 * b, N_tot) + 1):
+            for S2 in range(N % 2, min(N, 2 * b - N) + 1, 2):
+                ml = _mult_count(b, N, S2)
+                if ml <= 0:
+                    continue
+                mr = 0
+                for S2r in range(abs(S2 - S2_tot), S2 + S2_tot + 1, 2):
+                    mr += max(_mult_count(L - b, N_tot - N, S2r), 0)
+                if mr <= 0:
+                    continue
+                cand[(N, S2)] = (float(ml) * float(mr), min(ml, mr))
+        caps = {q: v[1] for q, v in cand.items()}
+        if sum(caps.values()) <= D:
+            secs.append(dict(caps))
+            continue
+        qs = sorted(cand)
+        w = np.array([cand[q][0] for q in qs], dtype=np.float64)
+        cap = np.array([cand[q][1] for q in qs], dtype=np.float64)
+        lo, hi = 0.0, float(D) / w.min() * 4.0
+        for _ in range(200):
+            mid = 0.5 * (lo + hi)
+            if np.minimum(cap, mid * w).sum() > D:
+                hi = mid
+            else:
+                lo = mid
+        x = np.minimum(cap, lo * w)
+        base = np.floor(x).astype(np.int64)
+        rem = x - base
+        short = int(D - base.sum())
+        order = np.argsort(-rem, kind="stable")
+        for idx in order[:max(short, 0)]:
+            if base[idx] < cap[idx]:
+                base[idx] += 1
+        secs.append({q: int(d) for q, d in zip(qs, base) if d > 0})
+    for _ in range(3):
+        for b in range(1, L + 1):
+            new = {}
+            for q, d in secs[b].items():
+                tot = 0
+                for qi, di in secs[b - 1].items():
+                    for m in range(3):
+                        if q in su2_couplings(qi, m):
+                            tot += di
+                d2 = min(d, tot)
+                if d2 > 0:
+                    new[q] = d2
+            secs[b] = new
+        for b in range(L - 1, -1, -1):
+            new = {}
+            for q, d in secs[b].items():
+                tot = 0
+                for m in range(3):
+                    for qo in su2_couplings(q, m):
+                        tot += secs[b + 1].get(qo, 0)
+                d2 = min(d, tot)
+                if d2 > 0:
+                    new[q] = d2
+            secs[b] = new
+    return secs
+
+
+@dataclass
+class SU2MPSInput:
+    """Random reduced (multiplet) MPS around the bond (k, k+1), total spin 0.
+
+    sectors[b] : dict (N, 2S) -> number of multiplets, label = content of sites 1..b (the right block of
+                 a bond then holds (N_tot - N, S), because S_tot = 0)
+    left[i]    : sites 1..k-1, dict (q_in, m, q_out) -> (d_in, d_out), sum over (q_in, m) of A^T A = 1 per q_out
+    right[i]   : sites k+2..L, dict (q_in, m, q_out) -> (d_in, d_out), sum over (m, q_out) of A A^T = 1 per q_in
+    Coupling order: left states |(block, site) S'>, right states |(site, block) S'>.
+    """
+    L: int
+    k: int
+    N: int
+    sectors: list
+    left: dict = field(default_factory=dict)
+    right: dict = field(default_factory=dict)
+
+
+def make_mps_su2(L: int, N_tot: int, D: int, k: int, seed: int, sectors=None) -> SU2MPSInput:
+    if sectors is None:
+        sectors = su2_bond_sectors(L, N_tot, 0, D)
+    rng = np.random.Generator(np.random.PCG64(seed + 15485863))
+    mps = SU2MPSInput(L=L, k=k, N=N_tot, sectors=sectors)
+    for i in range(1, k):
+        site = {}
+        for qo in sorted(sectors[i]):
+            do = sectors[i][qo]
+            rows = []
+            for qi in sorted(sectors[i - 1]):
+                for m in range(3):
+                    if qo in su2_couplings(qi, m):
+                        rows.append((qi, m, sectors[i - 1][qi]))
+            nrow = sum(r[2] for r in rows)
+            assert nrow >= do, "sector clipping failed (left, su2)"
+            Q, R = np.linalg.qr(rng.normal(size=(nrow, do)))
+            Q = Q * np.sign(np.diag(R))[None, :]
+            off = 0
+            for qi, m, d in rows:
+                site[(qi, m, qo)] = np.ascontiguousarray(Q[off:off + d, :])
+                off += d
+        mps.left[i] = site
+    for i in range(L, k + 1, -1):
+        site = {}
+        for qi in sorted(sectors[i - 1]):
+            di = sectors[i - 1][qi]
+            cols = []
+            for m in range(3):
+                for qo in su2_couplings(qi, m):
+                    if qo in sectors[i]:
+                        cols.append((m, qo, sectors[i][qo]))
+            ncol = sum(c[2] for c in cols)
+            assert ncol >= di, "sector clipping failed (right, su2)"
+            Q, R = np.linalg.qr(rng.normal(size=(ncol, di)))
+            Q = (Q * np.sign(np.diag(R))[None, :]).T
+            off = 0
+            for m, qo, d in cols:
+                site[(qi, m, qo)] = np.ascontiguousarray(Q[:, off:off + d])
+                off += d
+        mps.right[i] = site
+    return mps
+
+
+def psi_blocks_su2(mps: SU2MPSInput):
+    """Reduced two-site wavefunction blocks for S_tot = 0, in order (qL, m1, qLp, m2, qR):
+    qL = label of bond k-1, qLp = (N, 2S') of L' = L + site k, qR = label of bond k+1 (the right block holds
+    (N_tot - N, S) with that S), and R' = site k+1 + R must carry S' too, i.e. qLp in couplings(qL, m1) and
+    qR in couplings(qLp, m2).  Returns list of (qL, m1, qLp, m2, qR, dL, dR)."""
+    k = mps.k
+    sl, sr = mps.sectors[k - 1], mps.sectors[k + 1]
+    out = []
+    for qL in sorted(sl):
+        for m1 in range(3):
+            for qLp in sorted(su2_couplings(qL, m1)):
+                for m2 in range(3):
+                    for qR in sorted(su2_couplings(qLp, m2)):
+                        if qR in sr:
+                            out.append((qL, m1, qLp, m2, qR, sl[qL], sr[qR]))
+    return out
+
+
+def make_psi0_su2(mps: SU2MPSInput, seed: int):
+    rng = np.random.Generator(np.random.PCG64(seed + 32452843))
+    n = sum(b[5] * b[6] for b in psi_blocks_su2(mps))
+    v = rng.normal(size=n)
+    return v / np.linalg.norm(v)
+
+
+SU2_CONFIGS = {
+    3: dict(L=40, N=28, D=1024, ell=4.0, nP_per_L=2, seed=1003),
+    4: dict(L=56, N=40, D=4096, ell=12.0, nP_per_L=3, seed=1004),
+}
+
+
+def make_config_su2(cfg: int, D: int | None = None):
+    c = SU2_CONFIGS[cfg]
+    T, V = make_integrals(c["L"], c["seed"], c["ell"], c["nP_per_L"])
+    mps = make_mps_su2(c["L"], c["N"], c["D"] if D is None else D, c["L"] // 2, c["seed"])
+    return T, V, mps
