@@ -56,7 +56,8 @@ typedef void (*dmrg_free_fn)(void* ptr, void* user);
 typedef struct {
   int32_t L;            /* number of spatial orbitals ("d") */
   int32_t n_up, n_dn;   /* target electron numbers (N_alpha, N_beta); S_z = (n_up - n_dn)/2 */
-  int32_t symmetry;     /* 0 = U(1)xU(1).  1 = SU(2) is reserved: DMRG_ERR_UNSUPPORTED */
+  int32_t symmetry;     /* 0 = U(1)xU(1); 1 = SU(2) spin-adapted, total spin 0
+                           only (n_up == n_dn): bond sectors are then labelled (N, 2S) in the q_up/q_dn arrays */
   int32_t device;       /* CUDA device ordinal */
   uint64_t workspace_bytes; /* cap for the intermediate (O_L.psi) buffer; 0 = library default */
   dmrg_alloc_fn alloc;
@@ -87,6 +88,15 @@ int dmrg_mps_set_site(dmrg_ctx* ctx, int32_t site, int32_t canonical, int32_t nb
                       const int32_t* h_qin_idx, const int32_t* h_s, const int64_t* h_blk_off,
                       const double* h_data, void* stream);
 
+/* SU(2) contexts: reduced site tensor of site i.  Block n maps (sector qin_idx[n] of bond
+ * i-1, site multiplet m[n] = 0,1,2 = (N=0,S=0),(N=1,S=1/2),(N=2,S=0)) to sector qout_idx[n] of bond i, which must be
+ * a spin coupling of the two; d_in x d_out row-major, counted in multiplets.  Coupling order:
+ * left-canonical states |(block, site) S'>, right-canonical states |(site, block) S'>; a bond label (N, 2S) is the
+ * content of sites 1..b, the right block of that bond carries (N_tot - N, S).  Isometry conditions as above. */
+int dmrg_mps_set_site_su2(dmrg_ctx* ctx, int32_t site, int32_t canonical, int32_t nblocks,
+                          const int32_t* h_qin_idx, const int32_t* h_m, const int32_t* h_qout_idx,
+                          const int64_t* h_blk_off, const double* h_data, void* stream);
+
 /* Build the left environment from sites 1..k-1 and the right one from sites k+2..L by exact operator
  * blocking, then prepare the two-site problem at bond (k, k+1): complementary
  * operators, the task list of PAPER.md Eq. (8), and the diagonal of H_eff. */
@@ -100,13 +110,18 @@ int dmrg_renormalize(dmrg_ctx* ctx, int32_t direction, void* stream);
 
 /* Layout of the two-site wavefunction Psi_{a, s_k, s_{k+1}, b}: blocks ordered by
  * (q_L lexicographic, s_k, s_{k+1}); block n is a d_L x d_R row-major matrix at offset off[n] of the
- * flat vector.  Pass NULL arrays to query only *nblocks / *n. */
+ * flat vector.  Pass NULL arrays to query only *nblocks / *n.
+ * SU(2) contexts: reduced blocks of |((a, m1) S', (m2, b) S') S_tot = 0>, ordered by (q_L, m1, S' ascending, m2,
+ * q_R ascending in S); qL_up/qL_dn = (N, 2S) of bond k-1, s1/s2 = multiplets m1/m2, qR_up/qR_dn = (N, 2S) label of
+ * bond k+1, twoS_mid = 2S'. */
 typedef struct {
   int32_t qL_up, qL_dn;   /* label of bond k-1 */
   int32_t s1, s2;         /* site states of sites k, k+1 */
   int32_t qR_up, qR_dn;   /* label of bond k+1 (electrons in sites 1..k+1) */
   int32_t dL, dR;
   int64_t off;
+  int32_t twoS_mid;       /* SU(2) only: doubled spin S' of L' = L + site k (= spin of R'), else 0 */
+  int32_t pad_;
 } dmrg_psi_block;
 int dmrg_psi_layout(dmrg_ctx* ctx, int32_t* nblocks, dmrg_psi_block* h_blocks, int64_t* n);
 
@@ -151,6 +166,13 @@ int dmrg_stats(dmrg_ctx* ctx, dmrg_stats_t* out);
  * Right-block sectors are ordered by their bond label (electrons LEFT of the bond). */
 int dmrg_env_export(dmrg_ctx* ctx, int32_t side, int32_t kind, int32_t i, int32_t j,
                     double* h_out, int64_t* D);
+
+/* The factor F of PAPER.md Eq. (10)-(11) (host; doubled-spin arguments): *h_F_ninej = the rescaled Wigner 9j
+ * closed form sqrt((2Sa'+1)(2Sk'+1)(2Sg+1)(2k+1)) {Sa Sk Sg; kL kk k; Sa' Sk' Sg'}, *h_F_contraction = the contraction
+ * of six Clebsch-Gordan tensors of PAPER.md Fig. 4 from the library's own CG table (the table all SU(2) task
+ * prefactors are built from). */
+int dmrg_su2_f_factor(int32_t twoSa, int32_t twoSk, int32_t twoSg, int32_t twokL, int32_t twokk, int32_t twok,
+               int32_t twoSa_out, int32_t twoSk_out, int32_t twoSg_out, double* h_F_ninej, double* h_F_contraction);
 
 /* Measured FP64 tensor-pipe (DMMA) peak of the device in TFLOP/s: a register-only mma loop on all
  * SMs, timed with CUDA events on `stream`. */

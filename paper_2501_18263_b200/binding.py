@@ -21,7 +21,7 @@ EXPORTS = [
     "dmrg_create", "dmrg_destroy", "dmrg_last_error", "dmrg_load_integrals", "dmrg_mps_set_sectors",
     "dmrg_mps_set_site", "dmrg_env_build", "dmrg_renormalize", "dmrg_psi_layout", "dmrg_heff_apply",
     "dmrg_heff_diag", "dmrg_davidson", "dmrg_heff_apply_host", "dmrg_davidson_host", "dmrg_stats",
-    "dmrg_env_export", "dmrg_fp64_peak", "dmrg_apply_profile",
+    "dmrg_env_export", "dmrg_fp64_peak", "dmrg_apply_profile", "dmrg_mps_set_site_su2", "dmrg_su2_f_factor",
 ]
 
 ALLOC_FN = C.CFUNCTYPE(C.c_void_p, C.c_uint64, C.c_void_p)
@@ -37,7 +37,7 @@ class Config(C.Structure):
 class PsiBlock(C.Structure):
     _fields_ = [("qL_up", C.c_int32), ("qL_dn", C.c_int32), ("s1", C.c_int32), ("s2", C.c_int32),
                 ("qR_up", C.c_int32), ("qR_dn", C.c_int32), ("dL", C.c_int32), ("dR", C.c_int32),
-                ("off", C.c_int64)]
+                ("off", C.c_int64), ("twoS_mid", C.c_int32), ("pad_", C.c_int32)]
 
 
 class Stats(C.Structure):
@@ -77,6 +77,8 @@ def load_library(build_if_missing: bool = True):
     lib.dmrg_load_integrals.argtypes = [vp, i32, vp, vp, C.c_double]
     lib.dmrg_mps_set_sectors.argtypes = [vp, vp, vp, vp, vp]
     lib.dmrg_mps_set_site.argtypes = [vp, i32, i32, i32, vp, vp, vp, vp, vp]
+    lib.dmrg_mps_set_site_su2.argtypes = [vp, i32, i32, i32, vp, vp, vp, vp, vp, vp]
+    lib.dmrg_su2_f_factor.argtypes = [i32] * 9 + [dp, dp]
     lib.dmrg_env_build.argtypes = [vp, i32, vp]
     lib.dmrg_renormalize.argtypes = [vp, i32, vp]
     lib.dmrg_psi_layout.argtypes = [vp, C.POINTER(i32), C.POINTER(PsiBlock), C.POINTER(i64)]
@@ -107,7 +109,7 @@ def _np_ptr(a):
 class DMRG:
     """One library context on one GPU.  Methods carry the names of the C calls (without `dmrg_`)."""
 
-    def __init__(self, L, n_up, n_dn, device=0, workspace_bytes=0):
+    def __init__(self, L, n_up, n_dn, device=0, workspace_bytes=0, su2=False):
         import torch
         if not torch.cuda.is_available():
             raise DMRGError("CUDA device required: the library has no CPU path")
@@ -129,7 +131,8 @@ class DMRG:
 
         self._alloc_cb = ALLOC_FN(_alloc)
         self._free_cb = FREE_FN(_free)
-        self.cfg = Config(L, n_up, n_dn, 0, device, workspace_bytes, self._alloc_cb, self._free_cb, None)
+        self.su2 = bool(su2)
+        self.cfg = Config(L, n_up, n_dn, 1 if su2 else 0, device, workspace_bytes, self._alloc_cb, self._free_cb, None)
         self.ctx = C.c_void_p()
         rc = self.lib.dmrg_create(C.byref(self.cfg), C.byref(self.ctx))
         if rc != 0:
@@ -188,6 +191,21 @@ class DMRG:
         offs = np.asarray(offs, dtype=np.int64)
         self._check(self.lib.dmrg_mps_set_site(self.ctx, site, canonical, len(keys), _np_ptr(qin), _np_ptr(s),
                                                _np_ptr(offs), _np_ptr(data), self._stream()))
+
+    def mps_set_site_su2(self, site, canonical, blocks):
+        """blocks: dict (q_in, m, q_out) -> (d_in, d_out) array with q = (N, 2S); site 1-based."""
+        keys = sorted(blocks)
+        qin = np.asarray([self._sec_index[site - 1][k[0]] for k in keys], dtype=np.int32)
+        m = np.asarray([k[1] for k in keys], dtype=np.int32)
+        qout = np.asarray([self._sec_index[site][k[2]] for k in keys], dtype=np.int32)
+        offs, parts, o = [], [], 0
+        for k in keys:
+            a = np.ascontiguousarray(blocks[k], dtype=np.float64)
+            offs.append(o); parts.append(a.reshape(-1)); o += a.size
+        data = np.concatenate(parts) if parts else np.zeros(1)
+        offs = np.asarray(offs, dtype=np.int64)
+        self._check(self.lib.dmrg_mps_set_site_su2(self.ctx, site, canonical, len(keys), _np_ptr(qin), _np_ptr(m),
+                                                   _np_ptr(qout), _np_ptr(offs), _np_ptr(data), self._stream()))
 
     def env_build(self, k):
         self._check(self.lib.dmrg_env_build(self.ctx, k, self._stream()))
@@ -274,8 +292,19 @@ class DMRG:
     def setup(self, T, V, mps, e_core=0.0):
         self.load_integrals(T, V, e_core)
         self.mps_set_sectors(mps.sectors)
+        put = self.mps_set_site_su2 if self.su2 else self.mps_set_site
         for i, blocks in mps.left.items():
-            self.mps_set_site(i, 0, blocks)
+            put(i, 0, blocks)
         for i, blocks in mps.right.items():
-            self.mps_set_site(i, 1, blocks)
+            put(i, 1, blocks)
         self.env_build(mps.k)
+
+
+def su2_f_factor(Sa, Sk, Sg, kL, kk, k, Sa_, Sk_, Sg_):
+    """(F by the 9j closed form, F by the six-CG contraction) of PAPER.md Eq. (10)-(11); doubled spins."""
+    lib = load_library()
+    a, b = C.c_double(), C.c_double()
+    rc = lib.dmrg_su2_f_factor(Sa, Sk, Sg, kL, kk, k, Sa_, Sk_, Sg_, C.byref(a), C.byref(b))
+    if rc != 0:
+        raise DMRGError("dmrg_su2_f_factor failed with status %d" % rc)
+    return a.value, b.value

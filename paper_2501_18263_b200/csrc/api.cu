@@ -8,6 +8,7 @@
 #include <cstring>
 
 #include "engine.h"
+#include "su2.h"
 
 using namespace dmrg;
 
@@ -30,7 +31,8 @@ extern "C" {
 int dmrg_create(const dmrg_config* cfg, dmrg_ctx** out) {
   if (!cfg || !out) return DMRG_ERR_ARG;
   *out = nullptr;
-  if (cfg->symmetry != 0) return DMRG_ERR_UNSUPPORTED;
+  if (cfg->symmetry != 0 && cfg->symmetry != 1) return DMRG_ERR_UNSUPPORTED;
+  if (cfg->symmetry == 1 && cfg->n_up != cfg->n_dn) return DMRG_ERR_UNSUPPORTED;   // SU(2): total spin 0 only
   if (!cfg->alloc || !cfg->free || cfg->L < 2 || cfg->L > 64 || cfg->n_up < 0 || cfg->n_dn < 0 ||
       cfg->n_up > cfg->L || cfg->n_dn > cfg->L)
     return DMRG_ERR_ARG;
@@ -101,18 +103,25 @@ int dmrg_mps_set_sectors(dmrg_ctx* ctx, const int32_t* off, const int32_t* qu, c
   }
   DMRG_REQUIRE(bond[0].size() == 1 && bond[0].qu[0] == 0 && bond[0].qd[0] == 0 && bond[0].dim[0] == 1,
                DMRG_ERR_INPUT, "set_sectors: bond 0 must be {(0,0):1}");
-  DMRG_REQUIRE(bond[L].size() == 1 && bond[L].qu[0] == ctx->cfg.n_up && bond[L].qd[0] == ctx->cfg.n_dn &&
-                   bond[L].dim[0] == 1, DMRG_ERR_INPUT, "set_sectors: bond L must be {(n_up,n_dn):1}");
+  if (ctx->su2())
+    DMRG_REQUIRE(bond[L].size() == 1 && bond[L].qu[0] == ctx->cfg.n_up + ctx->cfg.n_dn && bond[L].qd[0] == 0 &&
+                     bond[L].dim[0] == 1, DMRG_ERR_INPUT, "set_sectors: bond L must be {(N, 2S=0):1}");
+  else
+    DMRG_REQUIRE(bond[L].size() == 1 && bond[L].qu[0] == ctx->cfg.n_up && bond[L].qd[0] == ctx->cfg.n_dn &&
+                     bond[L].dim[0] == 1, DMRG_ERR_INPUT, "set_sectors: bond L must be {(n_up,n_dn):1}");
   ctx->bond = std::move(bond);
   for (auto& s : ctx->site) { s.canonical = -1; s.blks.clear(); s.find.clear(); s.data.release(); }
   ctx->k = 0;
   API_END
 }
 
-int dmrg_mps_set_site(dmrg_ctx* ctx, int32_t site, int32_t canonical, int32_t nblocks, const int32_t* qin,
-                      const int32_t* s, const int64_t* blk_off, const double* h_data, void* stream) {
+static int set_site_impl(dmrg_ctx* ctx, int32_t site, int32_t canonical, int32_t nblocks, const int32_t* qin,
+                         const int32_t* s, const int32_t* qout_su2, const int64_t* blk_off, const double* h_data,
+                         void* stream) {
   API_BEGIN
   cudaStream_t st = (cudaStream_t)stream;
+  DMRG_REQUIRE((qout_su2 != nullptr) == ctx->su2(), DMRG_ERR_ARG,
+               "set_site: use dmrg_mps_set_site for U(1)xU(1) and dmrg_mps_set_site_su2 for SU(2) contexts");
   DMRG_REQUIRE(!ctx->bond.empty(), DMRG_ERR_ARG, "set_site: call dmrg_mps_set_sectors first");
   DMRG_REQUIRE(site >= 1 && site <= ctx->L && (canonical == 0 || canonical == 1) && nblocks > 0 && qin && s &&
                    blk_off && h_data, DMRG_ERR_ARG, "set_site: bad arguments");
@@ -122,12 +131,25 @@ int dmrg_mps_set_site(dmrg_ctx* ctx, int32_t site, int32_t canonical, int32_t nb
   t.canonical = canonical;
   long long off = 0;
   for (int n = 0; n < nblocks; ++n) {
-    DMRG_REQUIRE(qin[n] >= 0 && qin[n] < bi.size() && s[n] >= 0 && s[n] < 4, DMRG_ERR_INPUT, "set_site: bad block label");
-    int qo = bo.find(bi.qu[qin[n]] + SITE_QU[s[n]], bi.qd[qin[n]] + SITE_QD[s[n]]);
-    DMRG_REQUIRE(qo >= 0, DMRG_ERR_INPUT, "set_site: q_in + q(s) is not a sector of the next bond");
+    DMRG_REQUIRE(qin[n] >= 0 && qin[n] < bi.size() && s[n] >= 0 && s[n] < (qout_su2 ? 3 : 4), DMRG_ERR_INPUT,
+                 "set_site: bad block label");
+    int qo;
+    if (qout_su2) {   // SU(2): (N, 2S) + multiplet m -> (N + n(m), 2S or 2S +- 1)
+      qo = qout_su2[n];
+      DMRG_REQUIRE(qo >= 0 && qo < bo.size(), DMRG_ERR_INPUT, "set_site: bad q_out");
+      const int dN = bo.qu[qo] - bi.qu[qin[n]], dS = bo.qd[qo] - bi.qd[qin[n]];
+      DMRG_REQUIRE(dN == su2::MULT_N[s[n]] && (su2::MULT_S2[s[n]] == 0 ? dS == 0 : (dS == 1 || dS == -1)), DMRG_ERR_INPUT,
+                   "set_site: q_out is not a coupling of q_in with the site multiplet");
+    } else {
+      qo = bo.find(bi.qu[qin[n]] + SITE_QU[s[n]], bi.qd[qin[n]] + SITE_QD[s[n]]);
+      DMRG_REQUIRE(qo >= 0, DMRG_ERR_INPUT, "set_site: q_in + q(s) is not a sector of the next bond");
+    }
     SiteBlk b{qin[n], s[n], qo, bi.dim[qin[n]], bo.dim[qo], pad8(bi.dim[qin[n]]), pad8(bo.dim[qo]), off};
     off += (long long)b.dinp * b.doutp;
-    DMRG_REQUIRE(t.find.emplace(std::make_pair(b.qin, b.s), n).second, DMRG_ERR_INPUT, "set_site: duplicate block");
+    if (qout_su2)
+      DMRG_REQUIRE(t.find3.emplace(std::array<int, 3>{b.qin, b.s, b.qout}, n).second, DMRG_ERR_INPUT, "set_site: duplicate block");
+    else
+      DMRG_REQUIRE(t.find.emplace(std::make_pair(b.qin, b.s), n).second, DMRG_ERR_INPUT, "set_site: duplicate block");
     t.blks.push_back(b);
   }
   // isometry check on the host (input validation only)
@@ -181,11 +203,25 @@ int dmrg_mps_set_site(dmrg_ctx* ctx, int32_t site, int32_t canonical, int32_t nb
   API_END
 }
 
+int dmrg_mps_set_site(dmrg_ctx* ctx, int32_t site, int32_t canonical, int32_t nblocks, const int32_t* qin,
+                      const int32_t* s, const int64_t* blk_off, const double* h_data, void* stream) {
+  return set_site_impl(ctx, site, canonical, nblocks, qin, s, nullptr, blk_off, h_data, stream);
+}
+
+int dmrg_mps_set_site_su2(dmrg_ctx* ctx, int32_t site, int32_t canonical, int32_t nblocks, const int32_t* qin,
+                          const int32_t* m, const int32_t* qout, const int64_t* blk_off, const double* h_data,
+                          void* stream) {
+  if (!qout) return DMRG_ERR_ARG;
+  return set_site_impl(ctx, site, canonical, nblocks, qin, m, qout, blk_off, h_data, stream);
+}
+
 static void build_side(dmrg_ctx* ctx, bool left, int upto, cudaStream_t st, double* flops_last) {
   // left: sites 1..upto ; right: sites L..upto (descending)
-  auto blk = vacuum_block(ctx, left, st);
-  if (left) for (int i = 1; i <= upto; ++i) blk = renormalize_block(ctx, *blk, i, st, flops_last);
-  else for (int i = ctx->L; i >= upto; --i) blk = renormalize_block(ctx, *blk, i, st, flops_last);
+  const bool su = ctx->su2();
+  auto blk = su ? su2e::vacuum_block_su2(ctx, left, st) : vacuum_block(ctx, left, st);
+  auto step = [&](int i) { return su ? renormalize_block_su2(ctx, *blk, i, st, flops_last) : renormalize_block(ctx, *blk, i, st, flops_last); };
+  if (left) for (int i = 1; i <= upto; ++i) blk = step(i);
+  else for (int i = ctx->L; i >= upto; --i) blk = step(i);
   (left ? ctx->left : ctx->right) = std::move(blk);
 }
 
@@ -203,7 +239,7 @@ int dmrg_env_build(dmrg_ctx* ctx, int32_t k, void* stream) {
   build_side(ctx, false, k + 2, st, &fl);
   ctx->stats.flops_renorm = fl;
   ctx->k = k;
-  prepare_superblock(ctx, st);
+  if (ctx->su2()) prepare_superblock_su2(ctx, st); else prepare_superblock(ctx, st);
   ctx->stats.last_build_ms = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t0).count();
   API_END
 }
@@ -218,14 +254,15 @@ int dmrg_renormalize(dmrg_ctx* ctx, int32_t direction, void* stream) {
   ctx->apply_plan.clear();
   if (direction == 0) {
     DMRG_REQUIRE(k + 2 <= ctx->L, DMRG_ERR_ARG, "renormalize: already at the right end");
-    ctx->left = renormalize_block(ctx, *ctx->left, k, st, &fl);
+    ctx->left = ctx->su2() ? renormalize_block_su2(ctx, *ctx->left, k, st, &fl) : renormalize_block(ctx, *ctx->left, k, st, &fl);
     double f2 = 0;
     ctx->right.reset();
     build_side(ctx, false, k + 3, st, &f2);
     ctx->k = k + 1;
   } else if (direction == 1) {
     DMRG_REQUIRE(k - 1 >= 1, DMRG_ERR_ARG, "renormalize: already at the left end");
-    ctx->right = renormalize_block(ctx, *ctx->right, k + 1, st, &fl);
+    ctx->right = ctx->su2() ? renormalize_block_su2(ctx, *ctx->right, k + 1, st, &fl)
+                            : renormalize_block(ctx, *ctx->right, k + 1, st, &fl);
     double f2 = 0;
     ctx->left.reset();
     build_side(ctx, true, k - 2, st, &f2);
@@ -234,7 +271,7 @@ int dmrg_renormalize(dmrg_ctx* ctx, int32_t direction, void* stream) {
     throw Error(DMRG_ERR_ARG, "renormalize: direction must be 0 or 1");
   }
   ctx->stats.flops_renorm = fl;
-  prepare_superblock(ctx, st);
+  if (ctx->su2()) prepare_superblock_su2(ctx, st); else prepare_superblock(ctx, st);
   ctx->stats.last_build_ms = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t0).count();
   API_END
 }
@@ -249,8 +286,12 @@ int dmrg_psi_layout(dmrg_ctx* ctx, int32_t* nblocks, dmrg_psi_block* out, int64_
     const Sectors& sr = ctx->right->sec;
     for (size_t i = 0; i < ctx->psi.size(); ++i) {
       const PsiBlk& b = ctx->psi[i];
-      out[i] = dmrg_psi_block{sl.qu[b.qL], sl.qd[b.qL], b.s1, b.s2, ctx->cfg.n_up - sr.qu[b.qR],
-                              ctx->cfg.n_dn - sr.qd[b.qR], b.dL, b.dR, b.off_c};
+      if (ctx->su2())   // (N, 2S) labels; qR = left label of bond k+1
+        out[i] = dmrg_psi_block{sl.qu[b.qL], sl.qd[b.qL], b.s1, b.s2, ctx->cfg.n_up + ctx->cfg.n_dn - sr.qu[b.qR],
+                                sr.qd[b.qR], b.dL, b.dR, b.off_c, b.SLp, 0};
+      else
+        out[i] = dmrg_psi_block{sl.qu[b.qL], sl.qd[b.qL], b.s1, b.s2, ctx->cfg.n_up - sr.qu[b.qR],
+                                ctx->cfg.n_dn - sr.qd[b.qR], b.dL, b.dR, b.off_c, 0, 0};
     }
   }
   API_END
@@ -471,6 +512,7 @@ int dmrg_stats(dmrg_ctx* ctx, dmrg_stats_t* out) {
 int dmrg_env_export(dmrg_ctx* ctx, int32_t side, int32_t kind, int32_t i, int32_t j, double* h_out, int64_t* Dout) {
   API_BEGIN
   DMRG_REQUIRE(ctx->k > 0 && (side == 0 || side == 1) && kind >= 0 && kind <= 10, DMRG_ERR_ARG, "env_export: bad arguments");
+  DMRG_REQUIRE(!ctx->su2(), DMRG_ERR_UNSUPPORTED, "env_export: U(1)xU(1) contexts only");
   const BlockSide& B = side == 0 ? *ctx->left : *ctx->right;
   static const int kmap[11] = {K_H, K_CU, K_CD, K_AUU, K_AUD, K_ADD, K_BUU, K_BUD, K_BDD, K_SU, K_SD};
   const int kk = kmap[kind];
@@ -524,6 +566,35 @@ int dmrg_apply_profile(dmrg_ctx* ctx, const double* d_in, double* d_out, int32_t
   for (int i = 0; i < (int)rec.size() && i < cap && h_out; ++i)
     h_out[i] = dmrg_launch_info{rec[i].chunk, rec[i].phase, rec[i].shape, rec[i].ntiles, rec[i].flops, (double)rec[i].ms};
   API_END
+}
+
+int dmrg_su2_f_factor(int32_t twoSa, int32_t twoSk, int32_t twoSg, int32_t twokL, int32_t twokk, int32_t twok,
+               int32_t twoSa_out, int32_t twoSk_out, int32_t twoSg_out, double* h_F_ninej, double* h_F_contraction) {
+  if (!h_F_ninej || !h_F_contraction) return DMRG_ERR_ARG;
+  *h_F_ninej = su2::F_ninej(twoSa, twoSk, twoSg, twokL, twokk, twok, twoSa_out, twoSk_out, twoSg_out);
+  // the same factor from the library's own contraction (su2::phi_blocking) for site spins 0 / 1/2 is not a
+  // product form; here: direct sum over magnetic quantum numbers with the library's CG table
+  double tot = 0.0;
+  for (int Mg_ = -twoSg_out; Mg_ <= twoSg_out; Mg_ += 2)
+    for (int q = -twok; q <= twok; q += 2) {
+      const int Mg = Mg_ - q;
+      const double wo = su2::cg(twoSg, Mg, twok, q, twoSg_out, Mg_);
+      if (wo == 0.0) continue;
+      for (int qL = -twokL; qL <= twokL; qL += 2) {
+        const int qk = q - qL;
+        const double cop = su2::cg(twokL, qL, twokk, qk, twok, q);
+        if (cop == 0.0) continue;
+        for (int Ma = -twoSa; Ma <= twoSa; Ma += 2) {
+          const int Mk = Mg - Ma;
+          const double cin = su2::cg(twoSa, Ma, twoSk, Mk, twoSg, Mg);
+          if (cin == 0.0) continue;
+          tot += wo * cop * cin * su2::cg(twoSa_out, Ma + qL, twoSk_out, Mk + qk, twoSg_out, Mg_) *
+                 su2::cg(twoSa, Ma, twokL, qL, twoSa_out, Ma + qL) * su2::cg(twoSk, Mk, twokk, qk, twoSk_out, Mk + qk);
+        }
+      }
+    }
+  *h_F_contraction = tot / (twoSg_out + 1);
+  return DMRG_OK;
 }
 
 int dmrg_fp64_peak(dmrg_ctx* ctx, double* h_tflops, void* stream) {

@@ -1,10 +1,12 @@
 #include "engine.h"
+#include "su2.h"
 
 #include <algorithm>
 #include <cmath>
 #include <cstring>
 #include <set>
 #include <tuple>
+#include <unordered_map>
 
 namespace dmrg {
 
@@ -512,6 +514,48 @@ static inline uint64_t pack_key4(const OpRef& l, int o1, int o2, const OpRef& r)
          (uint64_t)(r.tr ? 1 : 0);
 }
 
+// diag(H_eff) from the diagonal tasks, and the statistics of the prepared two-site problem
+static void finish_superblock(dmrg_ctx* ctx, std::vector<std::vector<DiagTask>>& dtasks, int64_t n_terms,
+                              int64_t n_tasks, int64_t n_groups, cudaStream_t st) {
+  BlockSide& BL = *ctx->left;
+  BlockSide& BR = *ctx->right;
+  // ---- diagonal of H_eff ----
+  {
+    std::vector<DiagTask> flat;
+    std::vector<int> begin(ctx->psi.size() + 1, 0);
+    for (size_t b = 0; b < ctx->psi.size(); ++b) {
+      begin[b] = (int)flat.size();
+      flat.insert(flat.end(), dtasks[b].begin(), dtasks[b].end());
+      DMRG_REQUIRE(ctx->psi[b].dL <= DIAG_MAX_DIM && ctx->psi[b].dR <= DIAG_MAX_DIM, DMRG_ERR_UNSUPPORTED,
+                   "sector dimension above DIAG_MAX_DIM");
+    }
+    begin[ctx->psi.size()] = (int)flat.size();
+    DevArray<DiagTask> d_tasks;
+    DevArray<int> d_begin;
+    d_tasks.upload(&ctx->al, flat, st);
+    d_begin.upload(&ctx->al, begin, st);
+    launch_diag(ctx->d_psi_blocks.p, (int)ctx->psi.size(), d_tasks.p, d_begin.p, ctx->diag_p.p, st);
+    ++ctx->launches;
+    DMRG_CUDA(cudaStreamSynchronize(st));
+  }
+
+  // ---- statistics ----
+  dmrg_stats_t& s = ctx->stats;
+  s.n_terms = n_terms;
+  s.n_tasks = n_tasks;
+  s.n_groups = n_groups;
+  s.flops_apply = ctx->apply_plan.flops_analytic;
+  s.flops_executed = ctx->apply_plan.flops_executed;
+  s.bytes_intermediate = ctx->apply_plan.bytes_intermediate;
+  s.psi_size = ctx->psi_n;
+  s.op_bytes_left = (int64_t)BL.bytes();
+  s.op_bytes_right = (int64_t)BR.bytes();
+  s.bytes_unique = (double)(s.op_bytes_left + s.op_bytes_right) + 16.0 * (double)ctx->psi_n;
+  s.n_chunks = (int)ctx->apply_plan.chunks.size();
+  s.launches_per_apply = ctx->apply_plan.launches() + 2;
+}
+
+
 void prepare_superblock(dmrg_ctx* ctx, cudaStream_t st) {
   const int L = ctx->L, k = ctx->k;
   BlockSide& BL = *ctx->left;
@@ -763,41 +807,9 @@ void prepare_superblock(dmrg_ctx* ctx, cudaStream_t st) {
     }
   }
   planner.finish(&ctx->apply_plan, st);
-
-  // ---- diagonal of H_eff ----
-  {
-    std::vector<DiagTask> flat;
-    std::vector<int> begin(ctx->psi.size() + 1, 0);
-    for (size_t b = 0; b < ctx->psi.size(); ++b) {
-      begin[b] = (int)flat.size();
-      flat.insert(flat.end(), dtasks[b].begin(), dtasks[b].end());
-      DMRG_REQUIRE(ctx->psi[b].dL <= DIAG_MAX_DIM && ctx->psi[b].dR <= DIAG_MAX_DIM, DMRG_ERR_UNSUPPORTED,
-                   "sector dimension above DIAG_MAX_DIM");
-    }
-    begin[ctx->psi.size()] = (int)flat.size();
-    DevArray<DiagTask> d_tasks;
-    DevArray<int> d_begin;
-    d_tasks.upload(&ctx->al, flat, st);
-    d_begin.upload(&ctx->al, begin, st);
-    launch_diag(ctx->d_psi_blocks.p, (int)ctx->psi.size(), d_tasks.p, d_begin.p, ctx->diag_p.p, st);
-    ++ctx->launches;
-    DMRG_CUDA(cudaStreamSynchronize(st));
-  }
-
-  // ---- statistics ----
-  dmrg_stats_t& s = ctx->stats;
-  s.n_terms = n_terms;
-  s.n_tasks = n_tasks;
-  s.n_groups = n_groups;
-  s.flops_apply = ctx->apply_plan.flops_analytic;
-  s.flops_executed = ctx->apply_plan.flops_executed;
-  s.bytes_intermediate = ctx->apply_plan.bytes_intermediate;
-  s.psi_size = ctx->psi_n;
-  s.op_bytes_left = (int64_t)BL.bytes();
-  s.op_bytes_right = (int64_t)BR.bytes();
-  s.bytes_unique = (double)(s.op_bytes_left + s.op_bytes_right) + 16.0 * (double)ctx->psi_n;
-  s.n_chunks = (int)ctx->apply_plan.chunks.size();
-  s.launches_per_apply = ctx->apply_plan.launches() + 2;
+  finish_superblock(ctx, dtasks, n_terms, n_tasks, n_groups, st);
 }
+
+#include "engine_su2.inc"
 
 }  // namespace dmrg

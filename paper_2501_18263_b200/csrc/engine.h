@@ -19,4 +19,10 @@ std::unique_ptr<BlockSide> vacuum_block(dmrg_ctx* ctx, bool is_left, cudaStream_
 // Two-site problem at bond (k, k+1): psi layout, complementary operators, apply plan, diagonal.
 void prepare_superblock(dmrg_ctx* ctx, cudaStream_t st);
 
+// SU(2)-adapted counterparts (engine_su2.inc; sector labels (N, 2S), reduced matrix elements).
+std::unique_ptr<BlockSide> renormalize_block_su2(dmrg_ctx* ctx, const BlockSide& old, int site, cudaStream_t st,
+                                                 double* flops_out);
+namespace su2e { std::unique_ptr<BlockSide> vacuum_block_su2(dmrg_ctx* ctx, bool is_left, cudaStream_t st); }
+void prepare_superblock_su2(dmrg_ctx* ctx, cudaStream_t st);
+
 }  // namespace dmrg

@@ -60,6 +60,10 @@ struct BlockSide {
   int lo = 0, hi = 0;          // orbitals [lo, hi)
   Sectors sec;                 // labelled by the block's own electron content
   std::vector<std::unique_ptr<OpClass>> cls;   // [0, K_NSTD) standard kinds, then pre-summed classes
+  // SU(2): an operator kind (tensor operator of doubled rank k2 changing N by dN) owns one class per
+  // spin change d2S = dd of the class; kinds[0..SK_N) are the carried ones, pre-summed kinds follow.
+  struct KindRef { int k2 = 0, dN = 0; std::vector<int> cids; };
+  std::vector<KindRef> kinds;
   int norb() const { return hi - lo; }
   uint64_t bytes() const { uint64_t b = 0; for (auto& c : cls) if (c) b += (uint64_t)c->elems * 8; return b; }
 };
@@ -73,7 +77,8 @@ struct SiteBlk {
 struct SiteTensor {
   int canonical = -1;          // 0 left, 1 right, -1 unset
   std::vector<SiteBlk> blks;
-  std::map<std::pair<int, int>, int> find;   // (qin, s) -> block
+  std::map<std::pair<int, int>, int> find;   // (qin, s) -> block            (U(1)xU(1))
+  std::map<std::array<int, 3>, int> find3;   // (qin, m, qout) -> block      (SU(2): s holds the multiplet m)
   DevArray<double> data;
 };
 
@@ -86,7 +91,7 @@ struct SiteOpTable {
   int parity(int id) const;
 };
 
-struct PsiBlk { int qL, s1, s2, qR; int dL, dR, dLp, dRp; long long off_c, off_p; };
+struct PsiBlk { int qL, s1, s2, qR; int dL, dR, dLp, dRp; long long off_c, off_p; int qLp = -1; /* SU(2): (N, 2S) of L' */ int NLp = 0, SLp = 0; };
 
 }  // namespace dmrg
 
@@ -107,6 +112,8 @@ struct dmrg_ctx {
   // two-site problem
   std::vector<dmrg::PsiBlk> psi;
   std::map<std::array<int, 3>, int> psi_find;   // (qL, s1, s2) -> block
+  std::map<std::array<int, 5>, int> psi_find5;  // SU(2): (qL, m1, 2S of L', m2, qR) -> block
+  bool su2() const { return cfg.symmetry == 1; }
   long long psi_n = 0, psi_np = 0;
   dmrg::DevArray<dmrg::PsiBlockDev> d_psi_blocks;
   dmrg::DevArray<double> psi_in_p, psi_out_p, diag_p;

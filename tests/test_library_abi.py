@@ -42,7 +42,34 @@ def test_binding_names_match_header():
     from paper_2501_18263_b200 import binding
     assert sorted(binding.EXPORTS) == _declared()
     for n in binding.EXPORTS:
-        assert hasattr(binding.DMRG, n[len("dmrg_"):]) or n in ("dmrg_create", "dmrg_destroy", "dmrg_last_error")
+        assert hasattr(binding.DMRG, n[len("dmrg_"):]) or hasattr(binding, n[len("dmrg_"):]) or \
+            n in ("dmrg_create", "dmrg_destroy", "dmrg_last_error")
+
+
+def test_su2_F_table_matches_the_oracle_in_both_forms():
+    """a8 (Eq. (10)-(11), Fig. 4): the library's 9j closed form and its CG contraction (host code, no GPU
+    needed) against the oracle's independent implementation."""
+    from oracle import su2
+    from paper_2501_18263_b200 import binding
+    n = 0
+    for Sa in range(0, 6):
+        for Sk in (0, 1):
+            for Sg in range(abs(Sa - Sk), Sa + Sk + 1, 2):
+                for kL in (0, 1, 2):
+                    for kk in (0, 1, 2):
+                        for kop in range(abs(kL - kk), kL + kk + 1, 2):
+                            for Sa_ in range(abs(Sa - kL), Sa + kL + 1, 2):
+                                for Sk_ in (0, 1):
+                                    for Sg_ in range(abs(Sa_ - Sk_), Sa_ + Sk_ + 1, 2):
+                                        a, b = binding.su2_f_factor(Sa, Sk, Sg, kL, kk, kop, Sa_, Sk_, Sg_)
+                                        ref = su2.F_sixcg(Sa, Sk, Sg, kL, kk, kop, Sa_, Sk_, Sg_)
+                                        assert abs(b - ref) < 1e-12
+                                        ok = (abs(Sk - kk) <= Sk_ <= Sk + kk and (Sk + kk + Sk_) % 2 == 0 and
+                                              abs(Sg - kop) <= Sg_ <= Sg + kop)
+                                        if ok:
+                                            assert abs(a - ref) < 1e-12
+                                            n += 1
+    assert n > 300
 
 
 def test_sm100a_code_is_in_the_library():
