@@ -167,18 +167,26 @@ def run_ours(args):
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
 
     cfg = args.config
-    c = inputs.CONFIGS[cfg]
-    D = args.D if args.D else (c["D"] if cfg != 4 else c["D"])
+    su2 = args.su2 or cfg == 4          # config 4 exists in SU(2) form only (BASELINE.json configs[4])
+    c = inputs.SU2_CONFIGS[cfg] if su2 else inputs.CONFIGS[cfg]
+    D = args.D if args.D else c["D"]
     t0 = time.perf_counter()
-    T, V, mps = inputs.make_config(cfg, D=D)
-    d = DMRG(mps.L, mps.n_up, mps.n_dn, device=local, workspace_bytes=args.workspace_gb << 30)
+    dev = torch.device("cuda", local)
+    if su2:
+        T, V, mps = inputs.make_config_su2(cfg, D=D)
+        n_up = n_dn = mps.N // 2
+        psi0 = inputs.make_psi0_su2(mps, c["seed"])
+    else:
+        T, V, mps = inputs.make_config(cfg, D=D)
+        n_up, n_dn = mps.n_up, mps.n_dn
+        psi0 = inputs.make_psi0(mps, c["seed"])
+    d = DMRG(mps.L, n_up, n_dn, device=local, workspace_bytes=args.workspace_gb << 30, su2=su2)
     d.setup(T, V, mps)
     torch.cuda.synchronize()
     setup_s = time.perf_counter() - t0
     st = d.stats()
     n = d.psi_size()
-    dev = torch.device("cuda", local)
-    x = torch.from_numpy(inputs.make_psi0(mps, c["seed"])).to(dev)
+    x = torch.from_numpy(psi0).to(dev)
     y = torch.empty_like(x)
     peak_tf = d.fp64_peak()
     try:
@@ -239,7 +247,7 @@ def run_ours(args):
     dom_ms = sum(v[2] for v in dom.values())
 
     # ---- end to end through the host-buffer C call (pinned host psi in, psi out)
-    hx = torch.from_numpy(inputs.make_psi0(mps, c["seed"])).pin_memory()
+    hx = torch.from_numpy(psi0.copy()).pin_memory()
     hy = torch.empty_like(hx).pin_memory()
     hxn, hyn = hx.numpy(), hy.numpy()
     d.heff_apply_host(hxn, hyn)
@@ -274,8 +282,10 @@ def run_ours(args):
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
                 "warmup": args.warmup, "ms_per_step": ms_max, "higher_is_better": True, "scaling": "weak",
                 "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-                "config": {"workload": "BASELINE configs[%d]: L=%d, N=(%d,%d), U(1)xU(1), D=%d, middle bond (%d,%d), "
-                                       "one H_eff.psi per step" % (cfg, mps.L, mps.n_up, mps.n_dn, D, mps.k, mps.k + 1),
+                "config": {"workload": "BASELINE configs[%d]: L=%d, N=(%d,%d), %s, D=%d%s, middle bond (%d,%d), "
+                                       "one H_eff.psi per step" % (cfg, mps.L, n_up, n_dn,
+                                                                   "SU(2) S=0" if su2 else "U(1)xU(1)", D,
+                                                                   " multiplets" if su2 else "", mps.k, mps.k + 1),
                            "psi_size": n, "terms": st["n_terms"], "tasks": st["n_tasks"],
                            "flops_per_apply": st["flops_apply"], "operator_bytes": st["op_bytes_left"] + st["op_bytes_right"],
                            "l2": ("256 MB buffer rewritten between timed steps" if flush is not None
@@ -318,6 +328,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=3)
     ap.add_argument("--D", type=int, default=0)
+    ap.add_argument("--su2", action="store_true", help="SU(2)-adapted form of the config (configs 3 and 4)")
     ap.add_argument("--workspace-gb", type=int, default=0, dest="workspace_gb", help="0 = library default")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--quick", action="store_true", help="skip the Davidson / renormalisation extras")
