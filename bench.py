@@ -154,17 +154,14 @@ def run_reference(args):
 def run_ours(args):
     import torch
     import torch.distributed as dist
-    from paper_2501_18263_b200 import inputs
+    from paper_2501_18263_b200 import inputs, replicas
     from paper_2501_18263_b200.binding import DMRG
 
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    rank = int(os.environ.get("RANK", "0"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device (no CPU fallback)")
     torch.cuda.set_device(local)
-    if world > 1:
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    rank, world = replicas.init("nccl", torch.device("cuda", local))
 
     cfg = args.config
     su2 = args.su2 or cfg == 4          # config 4 exists in SU(2) form only (BASELINE.json configs[4])
@@ -195,8 +192,7 @@ def run_ours(args):
         hbm_peak = 6650.0   # fallback of /opt/skills/guides/B200_PROFILING.md
 
     def barrier():
-        if world > 1:
-            dist.barrier()
+        replicas.barrier(world)
         torch.cuda.synchronize()
 
     # ---- device-resident: K applies, each timed with its own CUDA events on the launching stream.  At
@@ -225,11 +221,8 @@ def run_ours(args):
     clocks = sampler.stop()
     launches = d.stats()["total_launches"] - l0
     ms = sum(a.elapsed_time(b) for a, b in evs) / args.steps
-    tmax = torch.tensor([ms], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
-    ms_max = float(tmax.item())
-    value = world * st["flops_apply"] / (ms_max * 1e-3) * 1e-9
+    ms_max, fl_per_s = replicas.aggregate_throughput(st["flops_apply"], ms, world, dev)
+    value = fl_per_s * 1e-9
 
     # ---- the dominant kernel alone: every launch of one more apply bracketed by events (serial order)
     _, rec = d.apply_profile(x, y)
@@ -258,10 +251,8 @@ def run_ours(args):
         d.heff_apply_host(hxn, hyn)
     torch.cuda.synchronize()
     e2e_ms = (time.perf_counter() - t1) / esteps * 1e3
-    te = torch.tensor([e2e_ms], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(te, op=dist.ReduceOp.MAX)
-    e2e_val = world * st["flops_apply"] / (float(te.item()) * 1e-3) * 1e-9
+    e2e_max, e2e_fl = replicas.aggregate_throughput(st["flops_apply"], e2e_ms, world, dev)
+    e2e_val = e2e_fl * 1e-9
 
     extra = {}
     if rank == 0 and not args.quick:
@@ -293,7 +284,7 @@ def run_ours(args):
                            "workspace_chunks": st["n_chunks"], "parallelism": "replicas" if world > 1 else "single"},
                 "clocks": clocks,
                 "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": 8 * n, "d2h_bytes_per_step": 8 * n,
-                        "ms_per_step": float(te.item())},
+                        "ms_per_step": e2e_max},
                 "gpu_launches": int(launches),
                 "roofline": {"bound": "tensor", "achieved": value / world * 1e-3, "peak": peak_tf, "unit": "TFLOP/s",
                              "frac": value / world * 1e-3 / peak_tf, "traffic": None,

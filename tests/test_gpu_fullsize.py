@@ -1,0 +1,85 @@
+"""Properties that hold at any size, checked at BASELINE.json's full sizes in the launch configuration bench.py
+times (the oracle cannot be run there; element-wise parity is covered at configs 0-1 and the small cases).
+`-m gpu`."""
+import os
+
+import numpy as np
+import pytest
+
+from paper_2501_18263_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+
+
+def _ctx(cfg, su2=False):
+    import torch
+    from paper_2501_18263_b200.binding import DMRG
+    if not torch.cuda.is_available():
+        pytest.fail("gpu-marked test needs a CUDA device")
+    if su2:
+        T, V, mps = inputs.make_config_su2(cfg)
+        d = DMRG(mps.L, mps.N // 2, mps.N // 2, su2=True)
+    else:
+        T, V, mps = inputs.make_config(cfg)
+        d = DMRG(mps.L, mps.n_up, mps.n_dn)
+    d.setup(T, V, mps)
+    return d
+
+
+def _properties(d, nsample, seed):
+    import torch
+    n = d.psi_size()
+    g = torch.Generator(device="cpu").manual_seed(seed)
+    x = torch.randn(n, dtype=torch.float64, generator=g).cuda()
+    y = torch.randn(n, dtype=torch.float64, generator=g).cuda()
+    hx, hy = d.heff_apply(x), d.heff_apply(y)
+    # H_eff is real symmetric (PAPER.md:39 Hermitian H projected by an isometry)
+    a, b = float(torch.dot(y, hx)), float(torch.dot(x, hy))
+    assert abs(a - b) <= 1e-11 * float(torch.linalg.norm(hx) * torch.linalg.norm(y))
+    # linearity and determinism: same input -> bit-identical output; H(2x - y) = 2Hx - Hy
+    assert torch.equal(d.heff_apply(x), hx)
+    z = d.heff_apply(2 * x - y)
+    assert float(torch.linalg.norm(z - (2 * hx - hy)) / torch.linalg.norm(z)) <= 1e-12
+    # the diagonal kernel agrees with the apply on sampled unit vectors
+    dg = d.heff_diag()
+    rng = np.random.default_rng(seed)
+    e = torch.zeros(n, dtype=torch.float64, device="cuda")
+    for j in rng.integers(0, n, size=nsample):
+        e[j] = 1.0
+        he = d.heff_apply(e)
+        assert abs(float(he[j]) - float(dg[j])) <= 1e-10 * max(1.0, abs(float(dg[j])))
+        e[j] = 0.0
+    return hx
+
+
+def test_config2_properties_and_stream_independence():
+    d = _ctx(2)
+    hx = _properties(d, 12, 1)
+    st = d.stats()
+    assert st["flops_apply"] > 1e11 and st["n_tasks"] > 1e6
+    d.close()
+    # the same plan with every launch in order on one stream gives the same bits (no atomics, fixed order)
+    os.environ["DMRG_B200_SERIAL"] = "1"
+    try:
+        d2 = _ctx(2)
+    finally:
+        del os.environ["DMRG_B200_SERIAL"]
+    import torch
+    g = torch.Generator(device="cpu").manual_seed(1)
+    x = torch.randn(d2.psi_size(), dtype=torch.float64, generator=g).cuda()
+    assert torch.equal(d2.heff_apply(x), hx)
+    d2.close()
+
+
+def test_config3_u1_d4096_properties():
+    """The configuration `bench.py` times by default (north_star target)."""
+    d = _ctx(3)
+    assert d.psi_size() == 8085937
+    _properties(d, 4, 2)
+    d.close()
+
+
+def test_config3_su2_1024_multiplets_properties():
+    d = _ctx(3, su2=True)
+    _properties(d, 8, 3)
+    d.close()

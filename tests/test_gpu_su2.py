@@ -137,3 +137,16 @@ def test_su2_renormalize_step_matches_oracle():
     assert d.psi_size() == orc.psi_size()
     assert _rel(_apply_gpu(d, v), orc.apply(v)) <= REL_L2
     d.close()
+
+
+def test_su2_medium_size_against_oracle():
+    """Several tiles per block and ragged tails: L = 12, 12 electrons, 90 multiplets (U(1)-equivalent ~ 300)."""
+    L, N, k, D = 12, 12, 6, 90
+    T, V = inputs.make_integrals(L, 123)
+    mps = inputs.make_mps_su2(L, N, D, k, seed=11)
+    orc = _oracle(T, V, mps)
+    d = _gpu(T, V, mps)
+    v = inputs.make_psi0_su2(mps, 6)
+    assert d.psi_size() == orc.psi_size()
+    assert _rel(_apply_gpu(d, v), orc.apply(v)) <= REL_L2
+    d.close()
