@@ -347,7 +347,7 @@ using S64x64   = Cfg<64, 64, 2, 2, 2, 4, 2>;   // 32x32
 using S64x128  = Cfg<64, 128, 1, 4, 2, 3, 2>;  // 64x32
 using S128x32  = Cfg<128, 32, 4, 1, 2, 4, 2>;  // 32x32
 using S128x64  = Cfg<128, 64, 2, 2, 2, 3, 2>;  // 64x32
-using S128x128 = Cfg<128, 128, 2, 4, 4, 4, 1>; // 64x32
+using S128x128 = Cfg<128, 128, 2, 4, 4, 5, 1>; // 64x32
 
 }  // namespace
 

@@ -1,6 +1,7 @@
 #include "plan.h"
 
 #include <algorithm>
+#include <cstdlib>
 #include <numeric>
 
 namespace dmrg {
@@ -31,7 +32,7 @@ namespace {
 // tile boundaries; keep >= 16 CTAs per resident slot for load balance.
 int tiles_per_cta(int shape, int ntiles) {
   const int slots = 148 * gemm_shape_ctas_per_sm(shape);
-  return std::max(1, std::min(8, ntiles / (slots * 16)));
+  return std::max(1, std::min(16, ntiles / (slots * 16)));
 }
 cudaError_t launch_shape(const Phase& ph, int s, cudaStream_t st) {
   return launch_grouped_gemm(s, ph.outs.p, ph.segs.p, ph.tiles[s].p, ph.ntiles[s], tiles_per_cta(s, ph.ntiles[s]), st);
@@ -248,6 +249,7 @@ void Planner::finish(Plan* plan, cudaStream_t st) {
   plan->ws_half = ws_max_;
   if (ws_max_ > 0) plan->workspace.allocate(al_, (size_t)ws_max_ * (two_halves ? 2 : 1));
   double* ws = plan->workspace.p;
+  if (std::getenv("DMRG_B200_PLAN_STATS")) plan->print_stats = true;
 
   // ---- split-K: heavy outputs are cut into parts along their (segment, repeat) list so that one launch
   // has several CTAs per SM of comparable length.  Part 0 accumulates into C; the others write partial
@@ -367,6 +369,7 @@ void Planner::finish(Plan* plan, cudaStream_t st) {
             tw[shape].push_back({GTile{(int)oi, b, r.first, c.first}, w});
             ph.shape_flops[shape] += 2.0 * ksum * std::min(GEMM_DIMS[r.second], o.M - r.first) *
                                      std::min(GEMM_DIMS[c.second], o.N - c.first);
+            ph.shape_flops_full[shape] += 2.0 * w;
           }
     }
     for (int s = 0; s < GEMM_NSHAPES; ++s) {
@@ -380,6 +383,7 @@ void Planner::finish(Plan* plan, cudaStream_t st) {
     ph.segs.upload(al_, segs, st);
   };
   plan->chunks.resize(chunks_.size());
+  struct PS { double act = 0, full = 0; long long tiles = 0; } ps[2][GEMM_NSHAPES];
   for (size_t c = 0; c < chunks_.size(); ++c) {
     double* wsc = ws + ((c & 1) ? ws_max_ : 0);   // chunk c works in workspace half c & 1
     build(chunks_[c].p1, plan->chunks[c].p1, wsc);
@@ -398,7 +402,20 @@ void Planner::finish(Plan* plan, cudaStream_t st) {
       plan->chunks[c].p2.red_max_batch = mb;
       if (!rd.empty()) plan->chunks[c].p2.red.upload(al_, rd, st);
     }
+    for (int p = 0; p < 2; ++p) {
+      const Phase& ph = p ? plan->chunks[c].p2 : plan->chunks[c].p1;
+      for (int sh = 0; sh < GEMM_NSHAPES; ++sh) {
+        ps[p][sh].act += ph.shape_flops[sh]; ps[p][sh].full += ph.shape_flops_full[sh]; ps[p][sh].tiles += ph.ntiles[sh];
+      }
+    }
   }
+  if (plan->print_stats)
+    for (int p = 0; p < 2; ++p)
+      for (int sh = 0; sh < GEMM_NSHAPES; ++sh)
+        if (ps[p][sh].tiles)
+          fprintf(stderr, "plan phase %d shape %dx%d tiles %lld flops %.4g full-tile flops %.4g (fill %.3f)\n", p + 1,
+                  GEMM_DIMS[sh / 3], GEMM_DIMS[sh % 3], ps[p][sh].tiles, ps[p][sh].act, ps[p][sh].full,
+                  ps[p][sh].act / ps[p][sh].full);
   chunks_.clear();
 }
 

@@ -44,6 +44,7 @@ struct Phase {
   DevArray<GTile> tiles[GEMM_NSHAPES];   // one tile list per tile shape, heaviest tiles first
   int ntiles[GEMM_NSHAPES] = {0, 0, 0, 0, 0, 0, 0, 0, 0};
   double shape_flops[GEMM_NSHAPES] = {0, 0, 0, 0, 0, 0, 0, 0, 0};   // flops the tiles of each launch execute
+  double shape_flops_full[GEMM_NSHAPES] = {0, 0, 0, 0, 0, 0, 0, 0, 0};   // same with every tile counted at its full BM x BN
   DevArray<RedDesc> red;                  // split-K partial sums to fold into the outputs afterwards
   int nred = 0, red_max_batch = 1;
   int launches() const { int n = nred > 0; for (int s = 0; s < GEMM_NSHAPES; ++s) n += ntiles[s] > 0; return n; }
@@ -71,6 +72,7 @@ struct LaunchRecord { int chunk, phase, shape, ntiles; double flops; float ms; }
 struct Plan {
   std::vector<Chunk> chunks;
   DevArray<double> workspace, scratch;
+  bool print_stats = false;   // DMRG_B200_PLAN_STATS: per-shape tile fill printed when a plan is built
   long long ws_half = 0;   // elements per workspace half (two halves when there are several chunks)
   double flops_analytic = 0, flops_executed = 0, bytes_intermediate = 0;
   int64_t n_items = 0, n_products = 0;
