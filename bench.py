@@ -268,6 +268,23 @@ def run_ours(args):
         extra["davidson"] = {"iters": it, "ms_per_iter": (time.perf_counter() - t2) * 1e3 / it, "energy": E, "resid": rn}
         extra["env_build"] = {"setup_s": setup_s, "last_build_ms": st["last_build_ms"],
                               "last_renorm_step_gflop": st["flops_renorm"] * 1e-9}
+        if cfg <= 2 and not su2:
+            # BASELINE configs[2]: Davidson to 1e-8 and one operator-renormalisation step (site k joins the left block)
+            z2 = 0.01 * x
+            z2[int(torch.argmin(dg))] += 1.0
+            z2 /= torch.linalg.norm(z2)
+            t3 = time.perf_counter()
+            E2, it2, rn2 = d.davidson(z2, tol=1e-8, max_iter=400, max_basis=20)
+            torch.cuda.synchronize()
+            extra["davidson_1e-8"] = {"iters": it2, "ms_total": (time.perf_counter() - t3) * 1e3, "energy": E2, "resid": rn2}
+            nxt = inputs.make_mps(mps.L, n_up, n_dn, D, mps.k + 1, c["seed"], sectors=mps.sectors)
+            d.mps_set_site(mps.k, 0, nxt.left[mps.k])
+            d.renormalize(0)
+            torch.cuda.synchronize()
+            s2 = d.stats()
+            extra["renormalize_step"] = {"ms": s2["renorm_ms"], "gflop": s2["flops_renorm"] * 1e-9,
+                                         "tflops": s2["flops_renorm"] / (s2["renorm_ms"] * 1e-3) * 1e-12,
+                                         "includes": "host planning of the step + all launches + sync"}
 
     if rank == 0:
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,

@@ -156,6 +156,7 @@ typedef struct {
   double last_build_ms;     /* host+device time of the last dmrg_env_build / dmrg_renormalize */
   double flops_renorm;      /* analytic flops of the last renormalisation step */
   int64_t total_launches;   /* kernels launched by this context so far */
+  double renorm_ms;         /* host+device time of the single blocking step of the last dmrg_renormalize */
 } dmrg_stats_t;
 int dmrg_stats(dmrg_ctx* ctx, dmrg_stats_t* out);
 

@@ -45,7 +45,8 @@ class Stats(C.Structure):
                 ("flops_apply", C.c_double), ("flops_executed", C.c_double), ("bytes_unique", C.c_double),
                 ("bytes_intermediate", C.c_double), ("psi_size", C.c_int64), ("op_bytes_left", C.c_int64),
                 ("op_bytes_right", C.c_int64), ("n_chunks", C.c_int32), ("launches_per_apply", C.c_int32),
-                ("last_build_ms", C.c_double), ("flops_renorm", C.c_double), ("total_launches", C.c_int64)]
+                ("last_build_ms", C.c_double), ("flops_renorm", C.c_double), ("total_launches", C.c_int64),
+                ("renorm_ms", C.c_double)]
 
     def as_dict(self):
         return {f: getattr(self, f) for f, _ in self._fields_}

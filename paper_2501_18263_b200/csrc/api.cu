@@ -254,15 +254,19 @@ int dmrg_renormalize(dmrg_ctx* ctx, int32_t direction, void* stream) {
   ctx->apply_plan.clear();
   if (direction == 0) {
     DMRG_REQUIRE(k + 2 <= ctx->L, DMRG_ERR_ARG, "renormalize: already at the right end");
+    auto r0 = std::chrono::steady_clock::now();
     ctx->left = ctx->su2() ? renormalize_block_su2(ctx, *ctx->left, k, st, &fl) : renormalize_block(ctx, *ctx->left, k, st, &fl);
+    ctx->stats.renorm_ms = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - r0).count();
     double f2 = 0;
     ctx->right.reset();
     build_side(ctx, false, k + 3, st, &f2);
     ctx->k = k + 1;
   } else if (direction == 1) {
     DMRG_REQUIRE(k - 1 >= 1, DMRG_ERR_ARG, "renormalize: already at the left end");
+    auto r0 = std::chrono::steady_clock::now();
     ctx->right = ctx->su2() ? renormalize_block_su2(ctx, *ctx->right, k + 1, st, &fl)
                             : renormalize_block(ctx, *ctx->right, k + 1, st, &fl);
+    ctx->stats.renorm_ms = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - r0).count();
     double f2 = 0;
     ctx->left.reset();
     build_side(ctx, true, k - 2, st, &f2);
