@@ -46,6 +46,9 @@ __device__ __forceinline__ void mbar_arrive(unsigned long long* bar) {
 __device__ __forceinline__ void cp_async16(void* smem, const void* gmem) {
   asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(smem_u32(smem)), "l"(gmem));
 }
+__device__ __forceinline__ void cp_async16s(unsigned smem_addr, const void* gmem) {
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(smem_addr), "l"(gmem));
+}
 // the mbarrier receives one (pre-counted) arrival once all prior cp.async of this thread have landed
 __device__ __forceinline__ void cp_async_arrive(unsigned long long* bar) {
   asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];\n" ::"r"(smem_u32(bar)) : "memory");
@@ -118,31 +121,54 @@ __device__ __forceinline__ long long seg_off(int x, int nr, unsigned inv, long l
 // BX = tile extent in the non-K dimension, ext = valid extent (multiple of 8), kv = valid k (8 or 16).
 //   xcontig == 0: element (x, k) at src[x*ld + k]  -> smem [x][k], pitch PK
 //   xcontig == 1: element (x, k) at src[k*ld + x]  -> smem [k][x], pitch BX + 4
+// A thread keeps its 16-byte column (K-contiguous) or its x position (X-contiguous) for the whole tile and
+// walks rows with constant strides, so a copy costs a compare, the cp.async and two adds.
 template <int BX, int NPT>
 __device__ __forceinline__ void produce_tile(double* sm, const double* base, int ld, int x0, int ext, int k0, int kv,
                                              int xcontig, int nr, unsigned inv, long long stride, int pt) {
-  constexpr int ITERS = (BX * KC / 2 + NPT - 1) / NPT;
   if (!xcontig) {
+    constexpr int RS = NPT / 8;                  // rows per pass
+    constexpr int ITERS = (BX + RS - 1) / RS;
+    const int kk = (pt & 7) * 2;
+    if (kk >= kv) return;
+    int x = pt >> 3;
+    unsigned s = smem_u32(sm + x * PK + kk);
+    if (nr == 0) {
+      const double* g = base + (long long)(x0 + x) * ld + (k0 + kk);
+      const long long gs = (long long)RS * ld;
 #pragma unroll
-    for (int it = 0; it < ITERS; ++it) {
-      int c = pt + it * NPT;
-      int x = c / (KC / 2), kk = (c % (KC / 2)) * 2;
-      if (x < ext && kk < kv) {
-        int loc;
-        long long o = seg_off(x0 + x, nr, inv, stride, loc);
-        cp_async16(sm + x * PK + kk, base + o + (long long)loc * ld + k0 + kk);
+      for (int it = 0; it < ITERS; ++it) {
+        if (x < ext) cp_async16s(s, g);
+        x += RS; s += RS * PK * 8; g += gs;
+      }
+    } else {
+#pragma unroll
+      for (int it = 0; it < ITERS; ++it) {
+        if (x < ext) {
+          int loc;
+          const long long o = seg_off(x0 + x, nr, inv, stride, loc);
+          cp_async16s(s, base + o + (long long)loc * ld + (k0 + kk));
+        }
+        x += RS; s += RS * PK * 8;
       }
     }
   } else {
+    constexpr int HX = BX / 2;                   // 16-byte columns per k row
+    static_assert(NPT % HX == 0, "producer threads must cover whole k rows");
+    constexpr int KS = NPT / HX;                 // k rows per pass
+    constexpr int ITERS = (KC + KS - 1) / KS;
+    const int xx = (pt % HX) * 2;
+    if (xx >= ext) return;
+    int kr = pt / HX;
+    int loc;
+    const long long o = seg_off(x0 + xx, nr, inv, stride, loc);
+    const double* g = base + o + (long long)(k0 + kr) * ld + loc;
+    const long long gs = (long long)KS * ld;
+    unsigned s = smem_u32(sm + kr * (BX + 4) + xx);
 #pragma unroll
     for (int it = 0; it < ITERS; ++it) {
-      int c = pt + it * NPT;
-      int kr = c / (BX / 2), xx = (c % (BX / 2)) * 2;
-      if (kr < kv && xx < ext) {
-        int loc;
-        long long o = seg_off(x0 + xx, nr, inv, stride, loc);
-        cp_async16(sm + kr * (BX + 4) + xx, base + o + (long long)(k0 + kr) * ld + loc);
-      }
+      if (kr < kv) cp_async16s(s, g);
+      kr += KS; s += KS * (BX + 4) * 8; g += gs;
     }
   }
 }
@@ -339,11 +365,11 @@ struct Cfg {
 };
 
 //                 BM   BN  WR WC NP ST MINB     warp tile
-using S32x32   = Cfg<32, 32, 1, 1, 1, 6, 4>;   // 32x32
-using S32x64   = Cfg<32, 64, 1, 2, 1, 6, 3>;   // 32x32
+using S32x32   = Cfg<32, 32, 1, 1, 2, 6, 4>;   // 32x32
+using S32x64   = Cfg<32, 64, 1, 2, 2, 6, 3>;   // 32x32
 using S32x128  = Cfg<32, 128, 1, 4, 2, 4, 2>;  // 32x32
-using S64x32   = Cfg<64, 32, 2, 1, 1, 6, 3>;   // 32x32
-using S64x64   = Cfg<64, 64, 2, 2, 2, 4, 2>;   // 32x32
+using S64x32   = Cfg<64, 32, 2, 1, 2, 6, 3>;   // 32x32
+using S64x64   = Cfg<64, 64, 2, 2, 4, 4, 2>;   // 32x32
 using S64x128  = Cfg<64, 128, 1, 4, 2, 3, 2>;  // 64x32
 using S128x32  = Cfg<128, 32, 4, 1, 2, 4, 2>;  // 32x32
 using S128x64  = Cfg<128, 64, 2, 2, 2, 3, 2>;  // 64x32
