@@ -174,7 +174,9 @@ __device__ __forceinline__ void produce_tile(double* sm, const double* base, int
 }
 
 // One pipeline stage of MMAs with compile-time shared-memory offsets.
-template <int BM, int BN, int FA, int FB, bool AX, bool BX, bool SCALE>
+// FAE x FBE (<= FA x FB) = the warp's 8x8 fragments that lie inside the tile's valid extent: a ragged tile
+// runs the variant with half the fragment rows and/or columns and pays tensor-pipe time for that area only.
+template <int BM, int BN, int FA, int FB, int FAE, int FBE, bool AX, bool BX, bool SCALE>
 __device__ __forceinline__ void compute_stage(double (&acc)[FA][FB][2], const double* sA, const double* sB,
                                               int wm0, int wn0, int lr, int lk, int kv, double alpha) {
   constexpr int SAM = AX ? 1 : PK, SAK = AX ? (BM + 4) : 1;
@@ -184,20 +186,35 @@ __device__ __forceinline__ void compute_stage(double (&acc)[FA][FB][2], const do
 #pragma unroll
   for (int kk = 0; kk < KC; kk += 4) {
     if (kk < kv) {
-      double af[FA], bf[FB];
+      double af[FAE], bf[FBE];
 #pragma unroll
-      for (int i = 0; i < FA; ++i) af[i] = pa[(8 * i) * SAM + kk * SAK];
+      for (int i = 0; i < FAE; ++i) af[i] = pa[(8 * i) * SAM + kk * SAK];
 #pragma unroll
-      for (int j = 0; j < FB; ++j) bf[j] = pb[(8 * j) * SBN + kk * SBK];
+      for (int j = 0; j < FBE; ++j) bf[j] = pb[(8 * j) * SBN + kk * SBK];
       if (SCALE) {
 #pragma unroll
-        for (int j = 0; j < FB; ++j) bf[j] *= alpha;
+        for (int j = 0; j < FBE; ++j) bf[j] *= alpha;
       }
 #pragma unroll
-      for (int i = 0; i < FA; ++i)
+      for (int i = 0; i < FAE; ++i)
 #pragma unroll
-        for (int j = 0; j < FB; ++j) dmma884(acc[i][j][0], acc[i][j][1], af[i], bf[j]);
+        for (int j = 0; j < FBE; ++j) dmma884(acc[i][j][0], acc[i][j][1], af[i], bf[j]);
     }
+  }
+}
+
+template <int BM, int BN, int FA, int FB, int FAE, int FBE>
+__device__ __forceinline__ void compute_dispatch(double (&acc)[FA][FB][2], const double* sA, const double* sB, int wm0,
+                                                 int wn0, int lr, int lk, int kv, double alpha, int flags) {
+  switch (flags & 7) {   // bit0 ta, bit1 tb, bit2 alpha != 1
+    case 0: compute_stage<BM, BN, FA, FB, FAE, FBE, false, true, false>(acc, sA, sB, wm0, wn0, lr, lk, kv, 1.0); break;
+    case 1: compute_stage<BM, BN, FA, FB, FAE, FBE, true, true, false>(acc, sA, sB, wm0, wn0, lr, lk, kv, 1.0); break;
+    case 2: compute_stage<BM, BN, FA, FB, FAE, FBE, false, false, false>(acc, sA, sB, wm0, wn0, lr, lk, kv, 1.0); break;
+    case 3: compute_stage<BM, BN, FA, FB, FAE, FBE, true, false, false>(acc, sA, sB, wm0, wn0, lr, lk, kv, 1.0); break;
+    case 4: compute_stage<BM, BN, FA, FB, FAE, FBE, false, true, true>(acc, sA, sB, wm0, wn0, lr, lk, kv, alpha); break;
+    case 5: compute_stage<BM, BN, FA, FB, FAE, FBE, true, true, true>(acc, sA, sB, wm0, wn0, lr, lk, kv, alpha); break;
+    case 6: compute_stage<BM, BN, FA, FB, FAE, FBE, false, false, true>(acc, sA, sB, wm0, wn0, lr, lk, kv, alpha); break;
+    default: compute_stage<BM, BN, FA, FB, FAE, FBE, true, false, true>(acc, sA, sB, wm0, wn0, lr, lk, kv, alpha); break;
   }
 }
 
@@ -290,12 +307,14 @@ k_grouped_gemm(const GOut* __restrict__ outs, const GSeg* __restrict__ segs, con
   double* C = nullptr;
   int ldc = 0, em = 0, en = 0, accum = 0;
   bool active = false;
+  int part = 0;
   while (true) {
     mbar_wait(&full_bar[stage], phase);
     const StageMeta mt = meta[stage];
     if (mt.flags & F_FIRST) {
       C = mt.C; ldc = mt.ldc; em = mt.em; en = mt.en; accum = mt.flags & F_ACC;
       active = wm0 < em && wn0 < en;   // warp-uniform
+      part = (em - wm0 <= 4 * FA ? 1 : 0) | (en - wn0 <= 4 * FB ? 2 : 0);
 #pragma unroll
       for (int i = 0; i < FA; ++i)
 #pragma unroll
@@ -304,15 +323,11 @@ k_grouped_gemm(const GOut* __restrict__ outs, const GSeg* __restrict__ segs, con
     if (active) {
       const double* sA = smem + stage * STAGE;
       const double* sB = sA + TA;
-      switch (mt.flags & 7) {
-        case 0: compute_stage<BM, BN, FA, FB, false, true, false>(acc, sA, sB, wm0, wn0, lr, lk, mt.kv, 1.0); break;
-        case 1: compute_stage<BM, BN, FA, FB, true, true, false>(acc, sA, sB, wm0, wn0, lr, lk, mt.kv, 1.0); break;
-        case 2: compute_stage<BM, BN, FA, FB, false, false, false>(acc, sA, sB, wm0, wn0, lr, lk, mt.kv, 1.0); break;
-        case 3: compute_stage<BM, BN, FA, FB, true, false, false>(acc, sA, sB, wm0, wn0, lr, lk, mt.kv, 1.0); break;
-        case 4: compute_stage<BM, BN, FA, FB, false, true, true>(acc, sA, sB, wm0, wn0, lr, lk, mt.kv, mt.alpha); break;
-        case 5: compute_stage<BM, BN, FA, FB, true, true, true>(acc, sA, sB, wm0, wn0, lr, lk, mt.kv, mt.alpha); break;
-        case 6: compute_stage<BM, BN, FA, FB, false, false, true>(acc, sA, sB, wm0, wn0, lr, lk, mt.kv, mt.alpha); break;
-        default: compute_stage<BM, BN, FA, FB, true, false, true>(acc, sA, sB, wm0, wn0, lr, lk, mt.kv, mt.alpha); break;
+      switch (part) {   // 0 full, 1 half the fragment rows, 2 half the columns, 3 both
+        case 0: compute_dispatch<BM, BN, FA, FB, FA, FB>(acc, sA, sB, wm0, wn0, lr, lk, mt.kv, mt.alpha, mt.flags); break;
+        case 1: compute_dispatch<BM, BN, FA, FB, FA / 2, FB>(acc, sA, sB, wm0, wn0, lr, lk, mt.kv, mt.alpha, mt.flags); break;
+        case 2: compute_dispatch<BM, BN, FA, FB, FA, FB / 2>(acc, sA, sB, wm0, wn0, lr, lk, mt.kv, mt.alpha, mt.flags); break;
+        default: compute_dispatch<BM, BN, FA, FB, FA / 2, FB / 2>(acc, sA, sB, wm0, wn0, lr, lk, mt.kv, mt.alpha, mt.flags); break;
       }
     }
     __syncwarp();
