@@ -278,7 +278,7 @@ void Planner::finish(Plan* plan, cudaStream_t st) {
       }
       mxa[i] = mx;
     }
-    const double wstar = total / (148.0 * 16.0);
+    const double wstar = total / (148.0 * 32.0);
     std::vector<HOut> ex;
     long long sc_used = 0;
     for (size_t i = 0; i < hv.size(); ++i) {
