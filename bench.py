@@ -145,7 +145,9 @@ def run_reference(args):
     line = {"impl": "reference", "metric": METRIC, "value": cb["value"], "unit": UNIT, "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": cb["ms_per_apply"], "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": "cpu oracle on a bounded sample: " + cb["sample"]},
+            "config": {"workload": "BASELINE configs[3] H_eff.psi (L=40, N=(14,14), U(1)xU(1), D=4096, middle bond); the CPU "
+                                   "oracle cannot finish that size in minutes, so each step is a bounded sample of the "
+                                   "same path on the same input recipe: " + cb["sample"]},
             "cpu_baseline": cb,
             "e2e": {"value": cb["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
     print(json.dumps(line))
