@@ -53,6 +53,11 @@ __device__ __forceinline__ void cp_async16s(unsigned smem_addr, const void* gmem
 __device__ __forceinline__ void cp_async_arrive(unsigned long long* bar) {
   asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];\n" ::"r"(smem_u32(bar)) : "memory");
 }
+__device__ __forceinline__ double lds64(unsigned addr) {
+  double v;
+  asm volatile("ld.shared.f64 %0, [%1];\n" : "=d"(v) : "r"(addr));
+  return v;
+}
 __device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double b) {
   asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
                : "+d"(c0), "+d"(c1)
@@ -181,16 +186,18 @@ __device__ __forceinline__ void compute_stage(double (&acc)[FA][FB][2], const do
                                               int wm0, int wn0, int lr, int lk, int kv, double alpha) {
   constexpr int SAM = AX ? 1 : PK, SAK = AX ? (BM + 4) : 1;
   constexpr int SBN = BX ? 1 : PK, SBK = BX ? (BN + 4) : 1;
-  const double* pa = sA + (wm0 + lr) * SAM + lk * SAK;
-  const double* pb = sB + (wn0 + lr) * SBN + lk * SBK;
+  // fragment loads as volatile asm: they keep their place before the (volatile) MMAs of the k-step, so the
+  // shared-memory latency is paid once per k-step instead of once per MMA
+  const unsigned pa = smem_u32(sA + (wm0 + lr) * SAM + lk * SAK);
+  const unsigned pb = smem_u32(sB + (wn0 + lr) * SBN + lk * SBK);
 #pragma unroll
   for (int kk = 0; kk < KC; kk += 4) {
     if (kk < kv) {
       double af[FAE], bf[FBE];
 #pragma unroll
-      for (int i = 0; i < FAE; ++i) af[i] = pa[(8 * i) * SAM + kk * SAK];
+      for (int i = 0; i < FAE; ++i) af[i] = lds64(pa + ((8 * i) * SAM + kk * SAK) * 8);
 #pragma unroll
-      for (int j = 0; j < FBE; ++j) bf[j] = pb[(8 * j) * SBN + kk * SBK];
+      for (int j = 0; j < FBE; ++j) bf[j] = lds64(pb + ((8 * j) * SBN + kk * SBK) * 8);
       if (SCALE) {
 #pragma unroll
         for (int j = 0; j < FBE; ++j) bf[j] *= alpha;
