@@ -60,6 +60,7 @@ typedef struct {
                            only (n_up == n_dn): bond sectors are then labelled (N, 2S) in the q_up/q_dn arrays */
   int32_t device;       /* CUDA device ordinal */
   uint64_t workspace_bytes; /* cap for the intermediate (O_L.psi) buffer; 0 = library default */
+  uint64_t env_cache_bytes; /* cap for cached environment blocks (sweeps re-use them); 0 = 1/8 of device memory */
   dmrg_alloc_fn alloc;
   dmrg_free_fn free;
   void* alloc_user;
@@ -97,6 +98,12 @@ int dmrg_mps_set_site_su2(dmrg_ctx* ctx, int32_t site, int32_t canonical, int32_
                           const int32_t* h_qin_idx, const int32_t* h_m, const int32_t* h_qout_idx,
                           const int64_t* h_blk_off, const double* h_data, void* stream);
 
+/* Replace the sectors of bond b (1 <= b <= L-1), e.g. after the SVD truncation of a sweep step changed the
+ * kept states.  Arrays as in dmrg_mps_set_sectors for that one bond (sorted).  The site tensors of sites b
+ * and b+1 and every cached environment that contains bond b become unset and must be given again. */
+int dmrg_mps_update_bond(dmrg_ctx* ctx, int32_t b, int32_t nsec, const int32_t* h_q_up, const int32_t* h_q_dn,
+                         const int32_t* h_dim);
+
 /* Build the left environment from sites 1..k-1 and the right one from sites k+2..L by exact operator
  * blocking, then prepare the two-site problem at bond (k, k+1): complementary
  * operators, the task list of PAPER.md Eq. (8), and the diagonal of H_eff. */
@@ -105,7 +112,8 @@ int dmrg_env_build(dmrg_ctx* ctx, int32_t k, void* stream);
 /* One renormalisation step: absorb site k into the left block (direction = 0, the
  * left-canonical tensor of site k must have been set) or site k+1 into the right block
  * (direction = 1), and prepare the two-site problem at the shifted bond (k+1,k+2) or (k-1,k).
- * The environment on the other side is rebuilt from the stored site tensors if needed. */
+ * The environment on the other side comes from the environment cache (blocks built earlier for the same site
+ * tensors) or is rebuilt from the stored site tensors. */
 int dmrg_renormalize(dmrg_ctx* ctx, int32_t direction, void* stream);
 
 /* Layout of the two-site wavefunction Psi_{a, s_k, s_{k+1}, b}: blocks ordered by

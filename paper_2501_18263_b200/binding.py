@@ -22,6 +22,7 @@ EXPORTS = [
     "dmrg_mps_set_site", "dmrg_env_build", "dmrg_renormalize", "dmrg_psi_layout", "dmrg_heff_apply",
     "dmrg_heff_diag", "dmrg_davidson", "dmrg_heff_apply_host", "dmrg_davidson_host", "dmrg_stats",
     "dmrg_env_export", "dmrg_fp64_peak", "dmrg_apply_profile", "dmrg_mps_set_site_su2", "dmrg_su2_f_factor",
+    "dmrg_mps_update_bond",
 ]
 
 ALLOC_FN = C.CFUNCTYPE(C.c_void_p, C.c_uint64, C.c_void_p)
@@ -30,7 +31,7 @@ FREE_FN = C.CFUNCTYPE(None, C.c_void_p, C.c_void_p)
 
 class Config(C.Structure):
     _fields_ = [("L", C.c_int32), ("n_up", C.c_int32), ("n_dn", C.c_int32), ("symmetry", C.c_int32),
-                ("device", C.c_int32), ("workspace_bytes", C.c_uint64), ("alloc", ALLOC_FN),
+                ("device", C.c_int32), ("workspace_bytes", C.c_uint64), ("env_cache_bytes", C.c_uint64), ("alloc", ALLOC_FN),
                 ("free", FREE_FN), ("alloc_user", C.c_void_p)]
 
 
@@ -78,6 +79,7 @@ def load_library(build_if_missing: bool = True):
     lib.dmrg_load_integrals.argtypes = [vp, i32, vp, vp, C.c_double]
     lib.dmrg_mps_set_sectors.argtypes = [vp, vp, vp, vp, vp]
     lib.dmrg_mps_set_site.argtypes = [vp, i32, i32, i32, vp, vp, vp, vp, vp]
+    lib.dmrg_mps_update_bond.argtypes = [vp, i32, i32, vp, vp, vp]
     lib.dmrg_mps_set_site_su2.argtypes = [vp, i32, i32, i32, vp, vp, vp, vp, vp, vp]
     lib.dmrg_su2_f_factor.argtypes = [i32] * 9 + [dp, dp]
     lib.dmrg_env_build.argtypes = [vp, i32, vp]
@@ -110,7 +112,7 @@ def _np_ptr(a):
 class DMRG:
     """One library context on one GPU.  Methods carry the names of the C calls (without `dmrg_`)."""
 
-    def __init__(self, L, n_up, n_dn, device=0, workspace_bytes=0, su2=False):
+    def __init__(self, L, n_up, n_dn, device=0, workspace_bytes=0, su2=False, env_cache_bytes=0):
         import torch
         if not torch.cuda.is_available():
             raise DMRGError("CUDA device required: the library has no CPU path")
@@ -133,7 +135,8 @@ class DMRG:
         self._alloc_cb = ALLOC_FN(_alloc)
         self._free_cb = FREE_FN(_free)
         self.su2 = bool(su2)
-        self.cfg = Config(L, n_up, n_dn, 1 if su2 else 0, device, workspace_bytes, self._alloc_cb, self._free_cb, None)
+        self.cfg = Config(L, n_up, n_dn, 1 if su2 else 0, device, workspace_bytes, env_cache_bytes, self._alloc_cb,
+                          self._free_cb, None)
         self.ctx = C.c_void_p()
         rc = self.lib.dmrg_create(C.byref(self.cfg), C.byref(self.ctx))
         if rc != 0:
@@ -178,6 +181,13 @@ class DMRG:
             off.append(len(qu))
         a = [np.asarray(x, dtype=np.int32) for x in (off, qu, qd, dim)]
         self._check(self.lib.dmrg_mps_set_sectors(self.ctx, *[_np_ptr(x) for x in a]))
+
+    def mps_update_bond(self, b, sectors):
+        """Replace the sectors of bond b by dict q -> dim (the site tensors b, b+1 must be set again)."""
+        keys = sorted(sectors)
+        self._sec_index[b] = {q: i for i, q in enumerate(keys)}
+        a = [np.asarray(x, dtype=np.int32) for x in ([q[0] for q in keys], [q[1] for q in keys], [sectors[q] for q in keys])]
+        self._check(self.lib.dmrg_mps_update_bond(self.ctx, b, len(keys), *[_np_ptr(x) for x in a]))
 
     def mps_set_site(self, site, canonical, blocks):
         """blocks: dict (q_in, s) -> (d_in, d_out) array, site 1-based, canonical 0 left / 1 right."""

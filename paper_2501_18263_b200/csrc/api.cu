@@ -83,6 +83,9 @@ int dmrg_load_integrals(dmrg_ctx* ctx, int32_t L, const double* h_T, const doubl
     ctx->w[((i * n + j) * n + k) * n + l] = 0.5 * (V(i, j, k, l) + V(j, i, l, k));
   ctx->e_core = e_core;
   ctx->have_integrals = true;
+  ctx->left_cache.clear(); ctx->right_cache.clear();   // every operator depends on the integrals
+  ctx->left.reset(); ctx->right.reset();
+  ctx->k = 0;
   API_END
 }
 
@@ -110,7 +113,9 @@ int dmrg_mps_set_sectors(dmrg_ctx* ctx, const int32_t* off, const int32_t* qu, c
     DMRG_REQUIRE(bond[L].size() == 1 && bond[L].qu[0] == ctx->cfg.n_up && bond[L].qd[0] == ctx->cfg.n_dn &&
                      bond[L].dim[0] == 1, DMRG_ERR_INPUT, "set_sectors: bond L must be {(n_up,n_dn):1}");
   ctx->bond = std::move(bond);
-  for (auto& s : ctx->site) { s.canonical = -1; s.blks.clear(); s.find.clear(); s.data.release(); }
+  for (auto& s : ctx->site) { s.canonical = -1; s.blks.clear(); s.find.clear(); s.find3.clear(); s.data.release(); }
+  ctx->left_cache.clear(); ctx->right_cache.clear();
+  ctx->left.reset(); ctx->right.reset();
   ctx->k = 0;
   API_END
 }
@@ -199,7 +204,29 @@ static int set_site_impl(dmrg_ctx* ctx, int32_t site, int32_t canonical, int32_t
   }
   t.data.upload(&ctx->al, padded, st);
   DMRG_CUDA(cudaStreamSynchronize(st));
+  ctx->invalidate_site(site);
   ctx->site[site] = std::move(t);
+  API_END
+}
+
+int dmrg_mps_update_bond(dmrg_ctx* ctx, int32_t b, int32_t nsec, const int32_t* qu, const int32_t* qd, const int32_t* dim) {
+  API_BEGIN
+  DMRG_REQUIRE(!ctx->bond.empty() && b >= 1 && b <= ctx->L - 1 && nsec > 0 && qu && qd && dim, DMRG_ERR_ARG,
+               "update_bond: bad arguments");
+  Sectors s;
+  for (int i = 0; i < nsec; ++i) {
+    DMRG_REQUIRE(dim[i] > 0 && qu[i] >= 0 && qd[i] >= 0, DMRG_ERR_INPUT, "update_bond: bad sector");
+    if (i > 0)
+      DMRG_REQUIRE(qu[i - 1] < qu[i] || (qu[i - 1] == qu[i] && qd[i - 1] < qd[i]), DMRG_ERR_INPUT, "update_bond: sectors not sorted");
+    s.add(qu[i], qd[i], dim[i]);
+  }
+  ctx->bond[b] = std::move(s);
+  for (int i : {b, b + 1}) {
+    SiteTensor& t = ctx->site[i];
+    t.canonical = -1; t.blks.clear(); t.find.clear(); t.find3.clear(); t.data.release();
+  }
+  ctx->invalidate_site(b);
+  ctx->invalidate_site(b + 1);
   API_END
 }
 
@@ -215,14 +242,38 @@ int dmrg_mps_set_site_su2(dmrg_ctx* ctx, int32_t site, int32_t canonical, int32_
   return set_site_impl(ctx, site, canonical, nblocks, qin, m, qout, blk_off, h_data, stream);
 }
 
+static uint64_t env_cache_cap(const dmrg_ctx* ctx) {
+  if (ctx->cfg.env_cache_bytes) return ctx->cfg.env_cache_bytes;
+  size_t fr = 0, tot = 0;
+  if (cudaMemGetInfo(&fr, &tot) != cudaSuccess) return 0;
+  return tot / 8;
+}
+
+static void cache_put(dmrg_ctx* ctx, bool left, int key, const std::shared_ptr<BlockSide>& b) {
+  if (ctx->cache_bytes() + b->bytes() > env_cache_cap(ctx)) return;
+  (left ? ctx->left_cache : ctx->right_cache)[key] = b;
+}
+
 static void build_side(dmrg_ctx* ctx, bool left, int upto, cudaStream_t st, double* flops_last) {
-  // left: sites 1..upto ; right: sites L..upto (descending)
+  // left: sites 1..upto ; right: sites L..upto (descending).  Starts from the nearest cached block.
   const bool su = ctx->su2();
-  auto blk = su ? su2e::vacuum_block_su2(ctx, left, st) : vacuum_block(ctx, left, st);
-  auto step = [&](int i) { return su ? renormalize_block_su2(ctx, *blk, i, st, flops_last) : renormalize_block(ctx, *blk, i, st, flops_last); };
-  if (left) for (int i = 1; i <= upto; ++i) blk = step(i);
-  else for (int i = ctx->L; i >= upto; --i) blk = step(i);
-  (left ? ctx->left : ctx->right) = std::move(blk);
+  std::shared_ptr<BlockSide> blk;
+  int from = left ? 0 : ctx->L + 1;     // block covers sites 1..from (left) or from..L (right)
+  if (left) {
+    for (auto& kv : ctx->left_cache) if (kv.first <= upto && kv.first >= from) { from = kv.first; blk = kv.second; }
+  } else {
+    for (auto& kv : ctx->right_cache) if (kv.first >= upto && kv.first <= from) { from = kv.first; blk = kv.second; }
+  }
+  if (!blk) blk = su ? su2e::vacuum_block_su2(ctx, left, st) : vacuum_block(ctx, left, st);
+  auto step = [&](int i) {
+    std::shared_ptr<BlockSide> nb = su ? renormalize_block_su2(ctx, *blk, i, st, flops_last)
+                                       : renormalize_block(ctx, *blk, i, st, flops_last);
+    cache_put(ctx, left, i, nb);
+    return nb;
+  };
+  if (left) for (int i = from + 1; i <= upto; ++i) blk = step(i);
+  else for (int i = from - 1; i >= upto; --i) blk = step(i);
+  (left ? ctx->left : ctx->right) = blk;
 }
 
 int dmrg_env_build(dmrg_ctx* ctx, int32_t k, void* stream) {
@@ -256,6 +307,7 @@ int dmrg_renormalize(dmrg_ctx* ctx, int32_t direction, void* stream) {
     DMRG_REQUIRE(k + 2 <= ctx->L, DMRG_ERR_ARG, "renormalize: already at the right end");
     auto r0 = std::chrono::steady_clock::now();
     ctx->left = ctx->su2() ? renormalize_block_su2(ctx, *ctx->left, k, st, &fl) : renormalize_block(ctx, *ctx->left, k, st, &fl);
+    cache_put(ctx, true, k, ctx->left);
     ctx->stats.renorm_ms = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - r0).count();
     double f2 = 0;
     ctx->right.reset();
@@ -266,6 +318,7 @@ int dmrg_renormalize(dmrg_ctx* ctx, int32_t direction, void* stream) {
     auto r0 = std::chrono::steady_clock::now();
     ctx->right = ctx->su2() ? renormalize_block_su2(ctx, *ctx->right, k + 1, st, &fl)
                             : renormalize_block(ctx, *ctx->right, k + 1, st, &fl);
+    cache_put(ctx, false, k + 1, ctx->right);
     ctx->stats.renorm_ms = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - r0).count();
     double f2 = 0;
     ctx->left.reset();

@@ -107,7 +107,20 @@ struct dmrg_ctx {
   std::vector<dmrg::Sectors> bond;          // bond sectors, label = electrons left of the bond
   std::vector<dmrg::SiteTensor> site;       // 1-based
   int k = 0;                                // current bond (k, k+1); 0 = none
-  std::unique_ptr<dmrg::BlockSide> left, right;
+  std::shared_ptr<dmrg::BlockSide> left, right;
+  // environment cache for sweeps: left_cache[i] = block of sites 1..i, right_cache[i] = block of sites i..L.
+  // Entries are dropped when a site tensor or bond they depend on changes; total size is capped.
+  std::map<int, std::shared_ptr<dmrg::BlockSide>> left_cache, right_cache;
+  uint64_t cache_bytes() const {
+    uint64_t b = 0;
+    for (auto& kv : left_cache) b += kv.second->bytes();
+    for (auto& kv : right_cache) b += kv.second->bytes();
+    return b;
+  }
+  void invalidate_site(int i) {     // site tensor i changed
+    for (auto it = left_cache.begin(); it != left_cache.end();) it = it->first >= i ? left_cache.erase(it) : std::next(it);
+    for (auto it = right_cache.begin(); it != right_cache.end();) it = it->first <= i ? right_cache.erase(it) : std::next(it);
+  }
   dmrg::SiteOpTable site_ops;
   // two-site problem
   std::vector<dmrg::PsiBlk> psi;

@@ -1,0 +1,157 @@
+"""Two-site DMRG sweep driver (SURVEY.md 8(f) item 1; Fig. 1, :63: eigensolve, SVD truncation,
+renormalisation, move on).  U(1)xU(1) contexts.
+
+Everything on the hot path runs in the library (`dmrg_davidson`, `dmrg_renormalize`, the environment cache).
+OUTSIDE the hot path, as north_star allows ("the truncation SVD is outside the hot path but stays on the
+device"), this driver does with torch on the device: the SVD of the optimised two-site tensor per middle-bond
+sector, the truncation to D states, and the wave-function transformation (next start vector).  The MPS
+tensors themselves are kept as host numpy blocks, because `dmrg_mps_set_site` takes host data.
+"""
+from __future__ import annotations
+
+import numpy as np
+
+SITE_Q = ((0, 0), (0, 1), (1, 0), (1, 1))
+
+
+def _qadd(q, s):
+    return (q[0] + SITE_Q[s][0], q[1] + SITE_Q[s][1])
+
+
+class TwoSiteSweep:
+    def __init__(self, d, T, V, mps, D, e_core=0.0):
+        """d: binding.DMRG (U(1)); mps: inputs.MPSInput positioned at bond (mps.k, mps.k+1)."""
+        self.d, self.D = d, D
+        self.L = mps.L
+        self.k = mps.k
+        self.sectors = [dict(s) for s in mps.sectors]
+        self.left = dict(mps.left)
+        self.right = dict(mps.right)
+        d.setup(T, V, mps, e_core)
+        self.guess = None
+        self.energies = []
+        self.trunc = []
+
+    # -- helpers --
+    def _layout(self):
+        blocks, n = self.d.psi_layout()
+        return [((b.qL_up, b.qL_dn), b.s1, b.s2, (b.qR_up, b.qR_dn), b.dL, b.dR, b.off) for b in blocks], n
+
+    def _start_vector(self, n, seed):
+        torch = self.d.torch
+        if self.guess is not None and self.guess.numel() == n:
+            return self.guess
+        g = torch.Generator(device="cpu").manual_seed(seed)
+        x = torch.randn(n, dtype=torch.float64, generator=g).to(self.d.device)
+        return x / torch.linalg.norm(x)
+
+    def step(self, direction, tol=1e-9, max_iter=200, max_basis=16, seed=0):
+        """Optimise the two-site tensor at the current bond, truncate, and move (0: right, 1: left, None: stay).
+        Returns the Davidson energy."""
+        torch = self.d.torch
+        d, k = self.d, self.k
+        layout, n = self._layout()
+        x = self._start_vector(n, seed).clone()
+        E, it, rn = d.davidson(x, tol=tol, max_iter=max_iter, max_basis=max_basis)
+        self.energies.append(E)
+        if direction is None:
+            self.guess = x
+            return E
+        # ---- SVD per middle-bond sector q_mid = qL + q(s1) ----
+        groups = {}
+        for (qL, s1, s2, qR, dL, dR, off) in layout:
+            g = groups.setdefault(_qadd(qL, s1), {"rows": {}, "cols": {}, "blk": []})
+            g["rows"].setdefault((qL, s1), dL)
+            g["cols"].setdefault((s2, qR), dR)
+            g["blk"].append(((qL, s1), (s2, qR), dL, dR, off))
+        svds, allsv = {}, []
+        for qm, g in groups.items():
+            ro, co, o = {}, {}, 0
+            for key in sorted(g["rows"]):
+                ro[key] = o; o += g["rows"][key]
+            nr, o = o, 0
+            for key in sorted(g["cols"]):
+                co[key] = o; o += g["cols"][key]
+            M = torch.zeros((nr, o), dtype=torch.float64, device=d.device)
+            for (rk, ck, dL, dR, off) in g["blk"]:
+                M[ro[rk]:ro[rk] + dL, co[ck]:co[ck] + dR] = x[off:off + dL * dR].view(dL, dR)
+            U, S, Vh = torch.linalg.svd(M, full_matrices=False)
+            svds[qm] = (U, S, Vh, ro, co, g)
+            allsv += [(float(s), qm) for s in S.cpu().numpy()]
+        allsv.sort(key=lambda t: -t[0])
+        kept = {}
+        for s, qm in allsv[:self.D]:
+            if s > 1e-14:
+                kept[qm] = kept.get(qm, 0) + 1
+        self.trunc.append(float(sum(s * s for s, _ in allsv[self.D:])))
+        new_sec = {qm: c for qm, c in kept.items()}
+        self.sectors[k] = new_sec
+        d.mps_update_bond(k, new_sec)
+        if direction == 0:
+            A, C = {}, {}
+            for qm, c in kept.items():
+                U, S, Vh, ro, co, g = svds[qm]
+                for (qL, s1), dL in g["rows"].items():
+                    A[(qL, s1)] = U[ro[(qL, s1)]:ro[(qL, s1)] + dL, :c].cpu().numpy()
+                C[qm] = (S[:c, None] * Vh[:c, :], co, g["cols"])
+            self.left[k] = A
+            d.mps_set_site(k, 0, A)
+            if k + 2 > self.L:
+                raise ValueError("already at the right end")
+            R = self.right.pop(k + 2)
+            d.renormalize(0)
+            self.k = k + 1
+            layout2, n2 = self._layout()
+            y = torch.zeros(n2, dtype=torch.float64, device=d.device)
+            for (qL, s1, s2, qR, dL, dR, off) in layout2:     # qL = q_mid, s1 = old s2, s2 = site k+2
+                if qL not in C:
+                    continue
+                Cm, co, cols = C[qL]
+                qmid2 = _qadd(qL, s1)
+                if (s1, qmid2) not in co or (qmid2, s2) not in R:
+                    continue
+                c0 = co[(s1, qmid2)]
+                w = cols[(s1, qmid2)]
+                Rb = torch.from_numpy(np.ascontiguousarray(R[(qmid2, s2)])).to(d.device)
+                y[off:off + dL * dR] = (Cm[:, c0:c0 + w] @ Rb).reshape(-1)
+        else:
+            B, C = {}, {}
+            for qm, c in kept.items():
+                U, S, Vh, ro, co, g = svds[qm]
+                for (s2, qR), dR in g["cols"].items():
+                    B[(qm, s2)] = Vh[:c, co[(s2, qR)]:co[(s2, qR)] + dR].cpu().numpy()
+                C[qm] = (U[:, :c] * S[None, :c], ro, g["rows"])
+            self.right[k + 1] = B
+            d.mps_set_site(k + 1, 1, B)
+            if k - 1 < 1:
+                raise ValueError("already at the left end")
+            Lt = self.left.pop(k - 1)
+            d.renormalize(1)
+            self.k = k - 1
+            layout2, n2 = self._layout()
+            y = torch.zeros(n2, dtype=torch.float64, device=d.device)
+            for (qL, s1, s2, qR, dL, dR, off) in layout2:     # s2 = old s1 (site k), qR = q_mid
+                if qR not in C:
+                    continue
+                Cm, ro, rows = C[qR]
+                qk1 = _qadd(qL, s1)                           # label of bond k-1
+                if (qk1, s2) not in ro or (qL, s1) not in Lt:
+                    continue
+                r0 = ro[(qk1, s2)]
+                h = rows[(qk1, s2)]
+                Lb = torch.from_numpy(np.ascontiguousarray(Lt[(qL, s1)])).to(d.device)
+                y[off:off + dL * dR] = (Lb @ Cm[r0:r0 + h, :]).reshape(-1)
+        nrm = torch.linalg.norm(y)
+        self.guess = y / nrm if float(nrm) > 0 else None
+        return E
+
+    def sweep(self, nsweeps=2, **kw):
+        """Right to the last bond, back to the first, ... starting from the current bond.  Returns energies."""
+        out = []
+        for _ in range(nsweeps):
+            while self.k + 2 <= self.L:
+                out.append(self.step(0, **kw))
+            while self.k - 1 >= 1:
+                out.append(self.step(1, **kw))
+        out.append(self.step(None, **kw))
+        return out
