@@ -2,6 +2,8 @@
 #include "su2.h"
 
 #include <algorithm>
+#include <chrono>
+#include <cstdlib>
 #include <cmath>
 #include <cstring>
 #include <set>
@@ -9,6 +11,20 @@
 #include <unordered_map>
 
 namespace dmrg {
+
+// DMRG_B200_TIMING=1: host-side phase times of the planning code on stderr (measurement aid)
+struct PhaseTimer {
+  bool on;
+  const char* what;
+  std::chrono::steady_clock::time_point t;
+  explicit PhaseTimer(const char* w) : on(std::getenv("DMRG_B200_TIMING") != nullptr), what(w), t(std::chrono::steady_clock::now()) {}
+  void lap(const char* name) {
+    if (!on) return;
+    auto n = std::chrono::steady_clock::now();
+    fprintf(stderr, "[timing] %s: %s %.1f ms\n", what, name, std::chrono::duration<double, std::milli>(n - t).count());
+    t = n;
+  }
+};
 
 // ------------------------------------------------------------------------------------------------
 // class storage
@@ -311,6 +327,7 @@ std::unique_ptr<BlockSide> renormalize_block(dmrg_ctx* ctx, const BlockSide& old
   }
   layout_standard(ctx, B, st);
 
+  PhaseTimer pt("renormalize");
   // ---- contributions: new operator = sum coef * (old operator (x) site operator) ----
   std::unordered_map<uint64_t, double> acc;
   auto in_old = [&](int orb) { return orb >= old.lo && orb < old.hi; };
@@ -410,6 +427,7 @@ std::unique_ptr<BlockSide> renormalize_block(dmrg_ctx* ctx, const BlockSide& old
     }
   }
 
+  pt.lap("enumerate strings");
   // ---- group by (dst kind, src class, transpose, site op), pre-sum where a destination has several sources
   struct GKey { int dk, sc, tr, sop; bool operator<(const GKey& o) const { return std::tie(dk, sc, tr, sop) < std::tie(o.dk, o.sc, o.tr, o.sop); } };
   std::map<GKey, std::vector<Entry>> groups;
@@ -441,6 +459,7 @@ std::unique_ptr<BlockSide> renormalize_block(dmrg_ctx* ctx, const BlockSide& old
   for (auto& f : fgs)
     for (auto& r : make_runs(f.e)) { cuts[f.g.dk].insert(r.a0); cuts[f.g.dk].insert(r.a0 + r.cnt); }
 
+  pt.lap("group + pre-sum");
   // ---- emit the triple products  new(q2' <- q1') += alpha * W2^T op(S)(q2 <- q1) W1 ----
   const uint64_t cap = workspace_cap(ctx);
   Planner planner(&ctx->al, cap);
@@ -497,10 +516,13 @@ std::unique_ptr<BlockSide> renormalize_block(dmrg_ctx* ctx, const BlockSide& old
       }
     }
   }
+  pt.lap("items");
   Plan plan;
   planner.finish(&plan, st);
+  pt.lap("planner.finish");
   plan.run(st, &ctx->launches, ctx->ex());
   DMRG_CUDA(cudaStreamSynchronize(st));
+  pt.lap("run");
   if (flops_out) *flops_out = plan.flops_analytic;
   return nb;
 }
@@ -599,6 +621,7 @@ void prepare_superblock(dmrg_ctx* ctx, cudaStream_t st) {
     DMRG_CUDA(cudaMemsetAsync(ctx->diag_p.p, 0, (size_t)std::max<long long>(op, 8) * 8, st));
   }
 
+  PhaseTimer pt("superblock");
   // ---- four-part terms  coef * O_L (x) o_1 (x) o_2 (x) O_R  of PAPER.md Eq. (6) ----
   std::unordered_map<uint64_t, double> acc;
   auto part_of = [&](int orb) { return orb < o_s1 ? 0 : (orb == o_s1 ? 1 : (orb == o_s2 ? 2 : 3)); };
@@ -674,6 +697,7 @@ void prepare_superblock(dmrg_ctx* ctx, cudaStream_t st) {
     }
   }
 
+  pt.lap("enumerate strings");
   // ---- group terms; pre-sum one side into complementary operators where that shortens the list ----
   struct GKey {
     int lc, lt, o1, o2, rc, rt;
@@ -719,6 +743,7 @@ void prepare_superblock(dmrg_ctx* ctx, cudaStream_t st) {
     fgs.push_back(std::move(f));
   }
   pre.run();
+  pt.lap("group + pre-sum");
 
   // ---- tasks of PAPER.md Eq. (8): (term group x psi block) -> contraction items + diagonal tasks ----
   const uint64_t cap = workspace_cap(ctx);
@@ -806,8 +831,11 @@ void prepare_superblock(dmrg_ctx* ctx, cudaStream_t st) {
       }
     }
   }
+  pt.lap("tasks -> items");
   planner.finish(&ctx->apply_plan, st);
+  pt.lap("planner.finish");
   finish_superblock(ctx, dtasks, n_terms, n_tasks, n_groups, st);
+  pt.lap("diag + stats");
 }
 
 #include "engine_su2.inc"
