@@ -1,17 +1,24 @@
 """Two-site DMRG sweep driver (SURVEY.md 8(f) item 1; Fig. 1, :63: eigensolve, SVD truncation,
-renormalisation, move on).  U(1)xU(1) contexts.
+renormalisation, move on).  U(1)xU(1) and SU(2) (total spin 0) contexts.
 
 Everything on the hot path runs in the library (`dmrg_davidson`, `dmrg_renormalize`, the environment cache).
 OUTSIDE the hot path, as north_star allows ("the truncation SVD is outside the hot path but stays on the
 device"), this driver does with torch on the device: the SVD of the optimised two-site tensor per middle-bond
 sector, the truncation to D states, and the wave-function transformation (next start vector).  The MPS
 tensors themselves are kept as host numpy blocks, because `dmrg_mps_set_site` takes host data.
+
+SU(2): the same steps on reduced (multiplet) blocks.  The middle-bond label of a block is (N, 2S') of
+L' = L + site k; the SVD factors are plain isometries on multiplets; a singular value is the total weight of
+its multiplet.  The wave-function transformation needs no extra factor: re-coupling
+|(a', (m2, (m3 b2)S_b) S') 0> -> |((a' m2) S_b, (m3 b2) S_b) 0> is a 6j symbol with a zero argument and equals +1
+(checked by the energy continuity test in tests/test_gpu_sweep.py).
 """
 from __future__ import annotations
 
 import numpy as np
 
 SITE_Q = ((0, 0), (0, 1), (1, 0), (1, 1))
+MULT_N = (0, 1, 2)
 
 
 def _qadd(q, s):
@@ -22,6 +29,7 @@ class TwoSiteSweep:
     def __init__(self, d, T, V, mps, D, e_core=0.0):
         """d: binding.DMRG (U(1)); mps: inputs.MPSInput positioned at bond (mps.k, mps.k+1)."""
         self.d, self.D = d, D
+        self.su2 = bool(getattr(d, "su2", False))
         self.L = mps.L
         self.k = mps.k
         self.sectors = [dict(s) for s in mps.sectors]
@@ -35,7 +43,19 @@ class TwoSiteSweep:
     # -- helpers --
     def _layout(self):
         blocks, n = self.d.psi_layout()
-        return [((b.qL_up, b.qL_dn), b.s1, b.s2, (b.qR_up, b.qR_dn), b.dL, b.dR, b.off) for b in blocks], n
+        out = []
+        for b in blocks:
+            qL, qR = (b.qL_up, b.qL_dn), (b.qR_up, b.qR_dn)
+            qm = (qL[0] + MULT_N[b.s1], b.twoS_mid) if self.su2 else _qadd(qL, b.s1)   # label of bond k
+            out.append((qL, b.s1, b.s2, qR, b.dL, b.dR, b.off, qm))
+        return out, n
+
+    def _lkey(self, qin, s, qout):
+        """Key of a site-tensor block (q_in, site state or multiplet[, q_out])."""
+        return (qin, s, qout) if self.su2 else (qin, s)
+
+    def _set_site(self, site, canonical, blocks):
+        (self.d.mps_set_site_su2 if self.su2 else self.d.mps_set_site)(site, canonical, blocks)
 
     def _start_vector(self, n, seed):
         torch = self.d.torch
@@ -59,8 +79,8 @@ class TwoSiteSweep:
             return E
         # ---- SVD per middle-bond sector q_mid = qL + q(s1) ----
         groups = {}
-        for (qL, s1, s2, qR, dL, dR, off) in layout:
-            g = groups.setdefault(_qadd(qL, s1), {"rows": {}, "cols": {}, "blk": []})
+        for (qL, s1, s2, qR, dL, dR, off, qm) in layout:
+            g = groups.setdefault(qm, {"rows": {}, "cols": {}, "blk": []})
             g["rows"].setdefault((qL, s1), dL)
             g["cols"].setdefault((s2, qR), dR)
             g["blk"].append(((qL, s1), (s2, qR), dL, dR, off))
@@ -92,10 +112,10 @@ class TwoSiteSweep:
             for qm, c in kept.items():
                 U, S, Vh, ro, co, g = svds[qm]
                 for (qL, s1), dL in g["rows"].items():
-                    A[(qL, s1)] = U[ro[(qL, s1)]:ro[(qL, s1)] + dL, :c].cpu().numpy()
+                    A[self._lkey(qL, s1, qm)] = U[ro[(qL, s1)]:ro[(qL, s1)] + dL, :c].cpu().numpy()
                 C[qm] = (S[:c, None] * Vh[:c, :], co, g["cols"])
             self.left[k] = A
-            d.mps_set_site(k, 0, A)
+            self._set_site(k, 0, A)
             if k + 2 > self.L:
                 raise ValueError("already at the right end")
             R = self.right.pop(k + 2)
@@ -103,26 +123,26 @@ class TwoSiteSweep:
             self.k = k + 1
             layout2, n2 = self._layout()
             y = torch.zeros(n2, dtype=torch.float64, device=d.device)
-            for (qL, s1, s2, qR, dL, dR, off) in layout2:     # qL = q_mid, s1 = old s2, s2 = site k+2
+            for (qL, s1, s2, qR, dL, dR, off, qmid2) in layout2:   # qL = old q_mid, s1 = old s2, s2 = site k+2
                 if qL not in C:
                     continue
                 Cm, co, cols = C[qL]
-                qmid2 = _qadd(qL, s1)
-                if (s1, qmid2) not in co or (qmid2, s2) not in R:
+                rk = self._lkey(qmid2, s2, qR)
+                if (s1, qmid2) not in co or rk not in R:
                     continue
                 c0 = co[(s1, qmid2)]
                 w = cols[(s1, qmid2)]
-                Rb = torch.from_numpy(np.ascontiguousarray(R[(qmid2, s2)])).to(d.device)
+                Rb = torch.from_numpy(np.ascontiguousarray(R[rk])).to(d.device)
                 y[off:off + dL * dR] = (Cm[:, c0:c0 + w] @ Rb).reshape(-1)
         else:
             B, C = {}, {}
             for qm, c in kept.items():
                 U, S, Vh, ro, co, g = svds[qm]
                 for (s2, qR), dR in g["cols"].items():
-                    B[(qm, s2)] = Vh[:c, co[(s2, qR)]:co[(s2, qR)] + dR].cpu().numpy()
+                    B[self._lkey(qm, s2, qR)] = Vh[:c, co[(s2, qR)]:co[(s2, qR)] + dR].cpu().numpy()
                 C[qm] = (U[:, :c] * S[None, :c], ro, g["rows"])
             self.right[k + 1] = B
-            d.mps_set_site(k + 1, 1, B)
+            self._set_site(k + 1, 1, B)
             if k - 1 < 1:
                 raise ValueError("already at the left end")
             Lt = self.left.pop(k - 1)
@@ -130,16 +150,16 @@ class TwoSiteSweep:
             self.k = k - 1
             layout2, n2 = self._layout()
             y = torch.zeros(n2, dtype=torch.float64, device=d.device)
-            for (qL, s1, s2, qR, dL, dR, off) in layout2:     # s2 = old s1 (site k), qR = q_mid
+            for (qL, s1, s2, qR, dL, dR, off, qk1) in layout2:   # s2 = old s1 (site k), qR = old q_mid, qk1 = bond k-1
                 if qR not in C:
                     continue
                 Cm, ro, rows = C[qR]
-                qk1 = _qadd(qL, s1)                           # label of bond k-1
-                if (qk1, s2) not in ro or (qL, s1) not in Lt:
+                lk = self._lkey(qL, s1, qk1)
+                if (qk1, s2) not in ro or lk not in Lt:
                     continue
                 r0 = ro[(qk1, s2)]
                 h = rows[(qk1, s2)]
-                Lb = torch.from_numpy(np.ascontiguousarray(Lt[(qL, s1)])).to(d.device)
+                Lb = torch.from_numpy(np.ascontiguousarray(Lt[lk])).to(d.device)
                 y[off:off + dL * dR] = (Lb @ Cm[r0:r0 + h, :]).reshape(-1)
         nrm = torch.linalg.norm(y)
         self.guess = y / nrm if float(nrm) > 0 else None

@@ -84,3 +84,50 @@ def test_environment_cache_is_reused_and_invalidated():
     d2.setup(T, V, a)
     assert steps < d2.stats()["total_launches"]
     d.close(); d2.close()
+
+
+def _sweeper_su2(L, N, D, seed, k0=1):
+    import torch
+    from paper_2501_18263_b200.binding import DMRG
+    from paper_2501_18263_b200.sweep import TwoSiteSweep
+    T, V = inputs.make_integrals(L, seed)
+    mps = inputs.make_mps_su2(L, N, D, k0, seed=seed)
+    d = DMRG(L, N // 2, N // 2, su2=True)
+    return TwoSiteSweep(d, T, V, mps, D), T, V
+
+
+@pytest.mark.parametrize("su2", [False, True])
+def test_wavefunction_transformation_keeps_the_energy(su2):
+    """Nothing discarded: the transformed start vector at the next bond is the same state, so its Rayleigh
+    quotient equals the energy just found (this also fixes the SU(2) re-coupling factor, +1)."""
+    import torch
+    sw, T, V = (_sweeper_su2(6, 6, 10 ** 9, 5, k0=2) if su2 else _sweeper(6, 3, 3, 10 ** 9, 5, k0=2))
+    for direction in (0, 0, 1, 1):
+        E = sw.step(direction, tol=1e-10, max_iter=300, max_basis=20)
+        g = sw.guess
+        assert abs(float(torch.linalg.norm(g)) - 1.0) < 1e-12
+        rq = float(torch.dot(g, sw.d.heff_apply(g)))
+        assert abs(rq - E) <= 1e-8, (direction, rq, E)
+    sw.d.close()
+
+
+def test_su2_sweep_reaches_the_fci_singlet():
+    sw, T, V = _sweeper_su2(6, 6, 10 ** 9, 5)
+    e_fci = fci.fci_lowest(T, V, 3, 3, 1)[0]          # singlet ground state for these integrals
+    es = sw.sweep(nsweeps=1, tol=1e-10, max_iter=300, max_basis=20)
+    assert max(abs(e - e_fci) for e in es[1:]) <= 1e-8
+    sw.d.close()
+    # L = 8, seed 1000: the FCI ground state of the S_z = 0 sector is a TRIPLET (-7.8244); the lowest singlet is
+    # the third FCI eigenvalue.  The SU(2) sweep (S = 0 sector only) must find exactly that one.
+    sw2, T2, V2 = _sweeper_su2(8, 8, 10 ** 9, 1000)
+    ev = fci.fci_lowest(T2, V2, 4, 4, 5)
+    es = sw2.sweep(nsweeps=1, tol=1e-10, max_iter=300, max_basis=20)
+    e_singlet = es[-1]
+    assert abs(e_singlet - ev[2]) <= 1e-7 and e_singlet > ev[0] + 1e-2
+    sw2.d.close()
+    # truncated to 20 multiplets: variational with respect to the singlet energy, and close to it
+    sw3, _, _ = _sweeper_su2(8, 8, 20, 1000)
+    es = sw3.sweep(nsweeps=2, tol=1e-9, max_iter=200, max_basis=16)
+    assert min(es[1:]) >= e_singlet - 1e-8
+    assert es[-1] - e_singlet <= 1e-2
+    sw3.d.close()
