@@ -47,6 +47,7 @@ int dmrg_create(const dmrg_config* cfg, dmrg_ctx** out) {
   c->al.user = cfg->alloc_user;
   c->L = cfg->L;
   c->site.resize(cfg->L + 2);
+  c->site_ops.build_products();
   try {
     if (!std::getenv("DMRG_B200_SERIAL")) c->exec.init();   // debugging aid: every launch in order on one stream
   } catch (const dmrg::Error&) {

@@ -102,7 +102,15 @@ int SiteOpTable::parity(int id) const {
 }
 
 // product of the elementary site operators in `ops` (leftmost first); returns interned id or -1
-static int site_product(SiteOpTable& tab, const EOp* ops, int n) {
+// product of the elementary site operators in `ops` (leftmost first); returns interned id or -1.
+// All strings of up to four elementary operators are interned when the table is built, so this is a
+// read-only lookup (the term enumeration calls it from several threads).
+static inline int site_code(const EOp* ops, int n) {
+  int code = 0, base = 0;
+  for (int i = 0; i < n; ++i) { code |= ((ops[i].cre ? 2 : 0) | ops[i].spin) << (2 * i); base = base * 4 + 1; }
+  return base + code;      // base = (4^n - 1) / 3
+}
+static int site_product_slow(SiteOpTable& tab, const EOp* ops, int n) {
   double m[16];
   std::memset(m, 0, sizeof(m));
   for (int i = 0; i < 4; ++i) m[i * 4 + i] = 1.0;
@@ -113,6 +121,16 @@ static int site_product(SiteOpTable& tab, const EOp* ops, int n) {
   }
   return tab.intern(m);
 }
+void SiteOpTable::build_products() {
+  prod.assign(341, -1);
+  for (int n = 0; n <= 4; ++n)
+    for (int c = 0; c < (1 << (2 * n)); ++c) {
+      EOp ops[4];
+      for (int i = 0; i < n; ++i) { int b = (c >> (2 * i)) & 3; ops[i] = EOp{(b & 2) != 0, 0, b & 1}; }
+      prod[site_code(ops, n)] = site_product_slow(*this, ops, n);
+    }
+}
+static inline int site_product(const SiteOpTable& tab, const EOp* ops, int n) { return tab.prod[site_code(ops, n)]; }
 
 // ------------------------------------------------------------------------------------------------
 // naming of block operators
@@ -629,7 +647,9 @@ void prepare_superblock(dmrg_ctx* ctx, cudaStream_t st) {
     if (o1 < 0 || o2 < 0 || coef == 0.0) return;
     acc[pack_key4(l, o1, o2, r)] += coef;
   };
-  auto add_ops = [&](const EOp* ops, int n, double coef) {
+  using AccMap = std::unordered_map<uint64_t, double>;
+  std::vector<AccMap> parts;
+  auto add_ops_to = [&](AccMap& m, const EOp* ops, int n, double coef, int* err) {
     EOp po[4][4];
     int np[4] = {0, 0, 0, 0}, inv = 0;
     for (int i = 0; i < n; ++i) {
@@ -640,13 +660,20 @@ void prepare_superblock(dmrg_ctx* ctx, cudaStream_t st) {
     OpRef l, r; double sl, sr;
     int rc = name_block_ops(BL, po[0], np[0], l, sl);
     if (rc == 1) return;
-    DMRG_REQUIRE(rc == 0, DMRG_ERR_ARG, "internal: unnamed left operator string");
+    if (rc != 0) { *err = 1; return; }
     rc = name_block_ops(BR, po[3], np[3], r, sr);
     if (rc == 1) return;
-    DMRG_REQUIRE(rc == 0, DMRG_ERR_ARG, "internal: unnamed right operator string");
-    int o1 = site_product(ctx->site_ops, po[1], np[1]);
-    int o2 = site_product(ctx->site_ops, po[2], np[2]);
-    add_named(l, o1, o2, r, coef * sl * sr * ((inv & 1) ? -1.0 : 1.0));
+    if (rc != 0) { *err = 1; return; }
+    const int o1 = site_product(ctx->site_ops, po[1], np[1]);
+    const int o2 = site_product(ctx->site_ops, po[2], np[2]);
+    const double c = coef * sl * sr * ((inv & 1) ? -1.0 : 1.0);
+    if (o1 < 0 || o2 < 0 || c == 0.0) return;
+    m[pack_key4(l, o1, o2, r)] += c;
+  };
+  auto add_ops = [&](const EOp* ops, int n, double coef) {
+    int err = 0;
+    add_ops_to(acc, ops, n, coef, &err);
+    DMRG_REQUIRE(!err, DMRG_ERR_ARG, "internal: unnamed operator string");
   };
   const OpRef ID{K_ID, 0, false};
   add_named(OpRef{K_H, 0, false}, 0, 0, ID, 1.0);
@@ -685,32 +712,72 @@ void prepare_superblock(dmrg_ctx* ctx, cudaStream_t st) {
       add_ops(o, 2, tv);
     }
   }
-  for (int i = 0; i < L; ++i) for (int j = 0; j < L; ++j) for (int kk = 0; kk < L; ++kk) for (int l = 0; l < L; ++l) {
-    int cnt[4] = {0, 0, 0, 0};
-    ++cnt[part_of(i)]; ++cnt[part_of(j)]; ++cnt[part_of(kk)]; ++cnt[part_of(l)];
-    if (cnt[0] >= 3 || cnt[3] >= 3) continue;                      // inside H^L/H^R or a+ S + h.c.
-    double wv = 0.5 * W4(ctx, i, j, kk, l);
-    if (wv == 0.0) continue;
-    for (int s = 0; s < 2; ++s) for (int t = 0; t < 2; ++t) {
-      EOp o[4] = {{true, i, s}, {true, j, t}, {false, l, t}, {false, kk, s}};
-      add_ops(o, 4, wv);
+  pt.lap("one-body + S strings");
+  // The L^4 two-body strings: eight buckets (i mod 8) with private maps, processed in parallel and merged
+  // in bucket order, so the coefficient sums do not depend on the number of threads.
+  {
+    constexpr int NB = 8;
+    std::vector<AccMap> loc(NB);
+    int err_any = 0;
+#pragma omp parallel for num_threads(NB) schedule(static, 1)
+    for (int b = 0; b < NB; ++b) {
+      int err = 0;
+      for (int i = b; i < L; i += NB)
+        for (int j = 0; j < L; ++j) for (int kk = 0; kk < L; ++kk) for (int l = 0; l < L; ++l) {
+          int cnt[4] = {0, 0, 0, 0};
+          ++cnt[part_of(i)]; ++cnt[part_of(j)]; ++cnt[part_of(kk)]; ++cnt[part_of(l)];
+          if (cnt[0] >= 3 || cnt[3] >= 3) continue;                      // inside H^L/H^R or a+ S + h.c.
+          const double wv = 0.5 * W4(ctx, i, j, kk, l);
+          if (wv == 0.0) continue;
+          for (int s = 0; s < 2; ++s) for (int t = 0; t < 2; ++t) {
+            EOp o[4] = {{true, i, s}, {true, j, t}, {false, l, t}, {false, kk, s}};
+            add_ops_to(loc[b], o, 4, wv, &err);
+          }
+        }
+      if (err) {
+#pragma omp atomic write
+        err_any = 1;
+      }
+    }
+    DMRG_REQUIRE(!err_any, DMRG_ERR_ARG, "internal: unnamed operator string");
+    pt.lap("two-body strings (parallel)");
+    // merge: partition p takes the keys with key % NB == p from every bucket map, in bucket order
+    parts.resize(NB);
+#pragma omp parallel for num_threads(NB) schedule(static, 1)
+    for (int p = 0; p < NB; ++p) {
+      AccMap& out = parts[p];
+      for (auto& kv : acc) if ((int)(kv.first % NB) == p) out[kv.first] += kv.second;   // one-body, S, H strings
+      for (int b = 0; b < NB; ++b)
+        for (auto& kv : loc[b]) if ((int)(kv.first % NB) == p) out[kv.first] += kv.second;
     }
   }
-
-  pt.lap("enumerate strings");
+  pt.lap("merge");
   // ---- group terms; pre-sum one side into complementary operators where that shortens the list ----
   struct GKey {
     int lc, lt, o1, o2, rc, rt;
     bool operator<(const GKey& o) const { return std::tie(lc, lt, o1, o2, rc, rt) < std::tie(o.lc, o.lt, o.o1, o.o2, o.rc, o.rt); }
   };
   std::map<GKey, std::vector<Entry>> groups;   // Entry: a = left index, b = right index
-  for (auto& kv : acc) {
-    if (std::fabs(kv.second) < 1e-300) continue;
-    uint64_t q = kv.first;
-    GKey g{(int)(q >> 50) & 63, (int)(q >> 37) & 1, (int)(q >> 28) & 511, (int)(q >> 19) & 511,
-           (int)(q >> 13) & 63, (int)(q & 1)};
-    groups[g].push_back(Entry{(int)(q >> 38) & 4095, (int)(q >> 1) & 4095, kv.second});
+  {
+    std::unordered_map<uint64_t, std::vector<Entry>*> fast;   // group bits of the key -> its entry list
+    const uint64_t gmask = ~((0xFFFull << 38) | (0xFFFull << 1));
+    for (auto& part : parts)
+      for (auto& kv : part) {
+        if (std::fabs(kv.second) < 1e-300) continue;
+        const uint64_t q = kv.first;
+        std::vector<Entry>*& v = fast[q & gmask];
+        if (!v) {
+          GKey g{(int)(q >> 50) & 63, (int)(q >> 37) & 1, (int)(q >> 28) & 511, (int)(q >> 19) & 511,
+                 (int)(q >> 13) & 63, (int)(q & 1)};
+          v = &groups[g];
+        }
+        v->push_back(Entry{(int)(q >> 38) & 4095, (int)(q >> 1) & 4095, kv.second});
+      }
+    // a fixed entry order inside every group (the partition maps iterate in hash order)
+    for (auto& kv : groups)
+      std::sort(kv.second.begin(), kv.second.end(), [](const Entry& x, const Entry& y) { return x.a != y.a ? x.a < y.a : x.b < y.b; });
   }
+  parts.clear();
   acc.clear();
   Presummer pre(ctx, st);
   struct FG { GKey g; int lcls, rcls; std::vector<Entry> e; };
@@ -718,11 +785,17 @@ void prepare_superblock(dmrg_ctx* ctx, cudaStream_t st) {
   int64_t n_terms = 0;
   for (auto& kv : groups) {
     FG f{kv.first, kv.first.lc, kv.first.rc, kv.second};
-    std::set<int> rows, cols;
-    for (auto& e : f.e) { rows.insert(e.a); cols.insert(e.b); }
+    size_t nrows = 0, ncols = 0;
+    {
+      std::vector<char> sr(4096, 0), sc(4096, 0);
+      for (auto& e : f.e) {
+        if (!sr[e.a]) { sr[e.a] = 1; ++nrows; }
+        if (!sc[e.b]) { sc[e.b] = 1; ++ncols; }
+      }
+    }
     const size_t nnz = f.e.size();
     const bool canL = f.g.lc != K_ID, canR = f.g.rc != K_ID;
-    size_t costL = canL ? cols.size() : nnz + 1, costR = canR ? rows.size() : nnz + 1;
+    size_t costL = canL ? ncols : nnz + 1, costR = canR ? nrows : nnz + 1;
     size_t best = std::min(costL, costR);
     if (best * 4 <= nnz * 3) {
       if (costL <= costR) {     // K^L[b] = sum_a coef * O_L[a]  for each right partner b

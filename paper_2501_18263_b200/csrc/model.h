@@ -86,6 +86,8 @@ struct OpRef { int cls = K_ID; int idx = 0; bool tr = false; };
 
 struct SiteOpTable {
   std::vector<std::array<double, 16>> mats;
+  std::vector<int> prod;       // id of every product of <= 4 elementary site operators (engine.cu site_code)
+  void build_products();
   SiteOpTable();
   int intern(const double* m);
   int parity(int id) const;

@@ -39,6 +39,15 @@ class TwoSiteSweep:
         self.guess = None
         self.energies = []
         self.trunc = []
+        # wall-time split per category, the ones of PAPER.md Fig. 20 (:284): Diag_H, SVD, Ren (+ Tables), StVec
+        self.seconds = {"Diag_H": 0.0, "SVD": 0.0, "Ren+Tables": 0.0, "StVec": 0.0}
+
+    def _tick(self, name, t0):
+        import time
+        self.d.torch.cuda.synchronize()
+        t1 = time.perf_counter()
+        self.seconds[name] += t1 - t0
+        return t1
 
     # -- helpers --
     def _layout(self):
@@ -71,8 +80,11 @@ class TwoSiteSweep:
         torch = self.d.torch
         d, k = self.d, self.k
         layout, n = self._layout()
+        import time
         x = self._start_vector(n, seed).clone()
+        t0 = time.perf_counter()
         E, it, rn = d.davidson(x, tol=tol, max_iter=max_iter, max_basis=max_basis)
+        t0 = self._tick("Diag_H", t0)
         self.energies.append(E)
         if direction is None:
             self.guess = x
@@ -104,6 +116,7 @@ class TwoSiteSweep:
             if s > 1e-14:
                 kept[qm] = kept.get(qm, 0) + 1
         self.trunc.append(float(sum(s * s for s, _ in allsv[self.D:])))
+        t0 = self._tick("SVD", t0)
         new_sec = {qm: c for qm, c in kept.items()}
         self.sectors[k] = new_sec
         d.mps_update_bond(k, new_sec)
@@ -121,6 +134,7 @@ class TwoSiteSweep:
             R = self.right.pop(k + 2)
             d.renormalize(0)
             self.k = k + 1
+            t0 = self._tick("Ren+Tables", t0)
             layout2, n2 = self._layout()
             y = torch.zeros(n2, dtype=torch.float64, device=d.device)
             for (qL, s1, s2, qR, dL, dR, off, qmid2) in layout2:   # qL = old q_mid, s1 = old s2, s2 = site k+2
@@ -148,6 +162,7 @@ class TwoSiteSweep:
             Lt = self.left.pop(k - 1)
             d.renormalize(1)
             self.k = k - 1
+            t0 = self._tick("Ren+Tables", t0)
             layout2, n2 = self._layout()
             y = torch.zeros(n2, dtype=torch.float64, device=d.device)
             for (qL, s1, s2, qR, dL, dR, off, qk1) in layout2:   # s2 = old s1 (site k), qR = old q_mid, qk1 = bond k-1
@@ -163,6 +178,7 @@ class TwoSiteSweep:
                 y[off:off + dL * dR] = (Lb @ Cm[r0:r0 + h, :]).reshape(-1)
         nrm = torch.linalg.norm(y)
         self.guess = y / nrm if float(nrm) > 0 else None
+        self._tick("StVec", t0)
         return E
 
     def sweep(self, nsweeps=2, **kw):
