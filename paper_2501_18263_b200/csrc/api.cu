@@ -85,6 +85,7 @@ int dmrg_load_integrals(dmrg_ctx* ctx, int32_t L, const double* h_T, const doubl
   ctx->e_core = e_core;
   ctx->have_integrals = true;
   ctx->left_cache.clear(); ctx->right_cache.clear();   // every operator depends on the integrals
+  ctx->term_cache.clear();
   ctx->left.reset(); ctx->right.reset();
   ctx->k = 0;
   API_END

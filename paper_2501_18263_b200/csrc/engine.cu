@@ -554,6 +554,18 @@ static inline uint64_t pack_key4(const OpRef& l, int o1, int o2, const OpRef& r)
          (uint64_t)(r.tr ? 1 : 0);
 }
 
+// Four-part term groups of one bond: (left class, transpose, site op 1, site op 2, right class, transpose) ->
+// coefficient entries (left operator, right operator, coefficient).  They depend on the bond and the
+// integrals only, so sweeps re-use them (dmrg_ctx::term_cache).
+struct TermGroups {
+  struct GKey {
+    int lc, lt, o1, o2, rc, rt;
+    bool operator<(const GKey& o) const { return std::tie(lc, lt, o1, o2, rc, rt) < std::tie(o.lc, o.lt, o.o1, o.o2, o.rc, o.rt); }
+  };
+  std::map<GKey, std::vector<Entry>> groups;
+  size_t bytes() const { size_t b = 0; for (auto& kv : groups) b += kv.second.size() * sizeof(Entry); return b; }
+};
+
 // diag(H_eff) from the diagonal tasks, and the statistics of the prepared two-site problem
 static void finish_superblock(dmrg_ctx* ctx, std::vector<std::vector<DiagTask>>& dtasks, int64_t n_terms,
                               int64_t n_tasks, int64_t n_groups, cudaStream_t st) {
@@ -640,145 +652,158 @@ void prepare_superblock(dmrg_ctx* ctx, cudaStream_t st) {
   }
 
   PhaseTimer pt("superblock");
-  // ---- four-part terms  coef * O_L (x) o_1 (x) o_2 (x) O_R  of PAPER.md Eq. (6) ----
-  std::unordered_map<uint64_t, double> acc;
-  auto part_of = [&](int orb) { return orb < o_s1 ? 0 : (orb == o_s1 ? 1 : (orb == o_s2 ? 2 : 3)); };
-  auto add_named = [&](const OpRef& l, int o1, int o2, const OpRef& r, double coef) {
-    if (o1 < 0 || o2 < 0 || coef == 0.0) return;
-    acc[pack_key4(l, o1, o2, r)] += coef;
-  };
-  using AccMap = std::unordered_map<uint64_t, double>;
-  std::vector<AccMap> parts;
-  auto add_ops_to = [&](AccMap& m, const EOp* ops, int n, double coef, int* err) {
-    EOp po[4][4];
-    int np[4] = {0, 0, 0, 0}, inv = 0;
-    for (int i = 0; i < n; ++i) {
-      int p = part_of(ops[i].orb);
-      for (int q = p + 1; q < 4; ++q) inv += np[q];   // operators of later parts already seen
-      po[p][np[p]++] = ops[i];
-    }
-    OpRef l, r; double sl, sr;
-    int rc = name_block_ops(BL, po[0], np[0], l, sl);
-    if (rc == 1) return;
-    if (rc != 0) { *err = 1; return; }
-    rc = name_block_ops(BR, po[3], np[3], r, sr);
-    if (rc == 1) return;
-    if (rc != 0) { *err = 1; return; }
-    const int o1 = site_product(ctx->site_ops, po[1], np[1]);
-    const int o2 = site_product(ctx->site_ops, po[2], np[2]);
-    const double c = coef * sl * sr * ((inv & 1) ? -1.0 : 1.0);
-    if (o1 < 0 || o2 < 0 || c == 0.0) return;
-    m[pack_key4(l, o1, o2, r)] += c;
-  };
-  auto add_ops = [&](const EOp* ops, int n, double coef) {
-    int err = 0;
-    add_ops_to(acc, ops, n, coef, &err);
-    DMRG_REQUIRE(!err, DMRG_ERR_ARG, "internal: unnamed operator string");
-  };
-  const OpRef ID{K_ID, 0, false};
-  add_named(OpRef{K_H, 0, false}, 0, 0, ID, 1.0);
-  add_named(ID, 0, 0, OpRef{K_H, 0, false}, 1.0);
-  for (int s = 0; s < 2; ++s) {
-    double mc[16], ma[16];
-    site_elem(true, s, mc);
-    site_elem(false, s, ma);
-    const int oc_ = ctx->site_ops.intern(mc), oa_ = ctx->site_ops.intern(ma);
-    const int sk = s == 0 ? K_SU : K_SD, ck = s == 0 ? K_CU : K_CD;
-    // x outside L:  a+_x S^L_x = - S^L_x a+_x ,  h.c. = (S^L_x)^T a_x
-    for (int x = o_s1; x < L; ++x) {
-      OpRef S{sk, idx_S(BL, x), false}, St{sk, idx_S(BL, x), true};
-      if (x == o_s1) { add_named(S, oc_, 0, ID, -1.0); add_named(St, oa_, 0, ID, 1.0); }
-      else if (x == o_s2) { add_named(S, 0, oc_, ID, -1.0); add_named(St, 0, oa_, ID, 1.0); }
-      else { add_named(S, 0, 0, OpRef{ck, x - BR.lo, false}, -1.0); add_named(St, 0, 0, OpRef{ck, x - BR.lo, true}, 1.0); }
-    }
-    // x outside R:  a+_x S^R_x ,  h.c. = (S^R_x)^T a_x = - a_x (S^R_x)^T
-    for (int x = 0; x <= o_s2; ++x) {
-      OpRef S{sk, idx_S(BR, x), false}, St{sk, idx_S(BR, x), true};
-      if (x == o_s1) { add_named(ID, oc_, 0, S, 1.0); add_named(ID, oa_, 0, St, -1.0); }
-      else if (x == o_s2) { add_named(ID, 0, oc_, S, 1.0); add_named(ID, 0, oa_, St, -1.0); }
-      else { add_named(OpRef{ck, x - BL.lo, false}, 0, 0, S, 1.0); add_named(OpRef{ck, x - BL.lo, true}, 0, 0, St, -1.0); }
-    }
-  }
-  auto is_block = [&](int p) { return p == 0 || p == 3; };
-  for (int i = 0; i < L; ++i) for (int j = 0; j < L; ++j) {
-    int pi = part_of(i), pj = part_of(j);
-    if (pi == pj && is_block(pi)) continue;                        // inside H^L / H^R
-    double f = 1.0;
-    if (pi != pj) f -= 0.5 * (is_block(pi) ? 1 : 0) + 0.5 * (is_block(pj) ? 1 : 0);   // halves carried by S^L, S^R
-    double tv = f * T2(ctx, i, j);
-    if (tv == 0.0) continue;
-    for (int s = 0; s < 2; ++s) {
-      EOp o[2] = {{true, i, s}, {false, j, s}};
-      add_ops(o, 2, tv);
-    }
-  }
-  pt.lap("one-body + S strings");
-  // The L^4 two-body strings: eight buckets (i mod 8) with private maps, processed in parallel and merged
-  // in bucket order, so the coefficient sums do not depend on the number of threads.
+  using GKey = TermGroups::GKey;
+  // The term groups depend on the bond and the integrals only: a sweep that comes back to this bond re-uses them.
+  std::shared_ptr<TermGroups> tg;
   {
-    constexpr int NB = 8;
-    std::vector<AccMap> loc(NB);
-    int err_any = 0;
-#pragma omp parallel for num_threads(NB) schedule(static, 1)
-    for (int b = 0; b < NB; ++b) {
+    auto f = ctx->term_cache.find(k);
+    if (f != ctx->term_cache.end()) tg = std::static_pointer_cast<TermGroups>(f->second);
+  }
+  if (!tg) {
+    // ---- four-part terms  coef * O_L (x) o_1 (x) o_2 (x) O_R  of PAPER.md Eq. (6) ----
+    std::unordered_map<uint64_t, double> acc;
+    auto part_of = [&](int orb) { return orb < o_s1 ? 0 : (orb == o_s1 ? 1 : (orb == o_s2 ? 2 : 3)); };
+    auto add_named = [&](const OpRef& l, int o1, int o2, const OpRef& r, double coef) {
+      if (o1 < 0 || o2 < 0 || coef == 0.0) return;
+      acc[pack_key4(l, o1, o2, r)] += coef;
+    };
+    using AccMap = std::unordered_map<uint64_t, double>;
+    std::vector<AccMap> parts;
+    auto add_ops_to = [&](AccMap& m, const EOp* ops, int n, double coef, int* err) {
+      EOp po[4][4];
+      int np[4] = {0, 0, 0, 0}, inv = 0;
+      for (int i = 0; i < n; ++i) {
+        int p = part_of(ops[i].orb);
+        for (int q = p + 1; q < 4; ++q) inv += np[q];   // operators of later parts already seen
+        po[p][np[p]++] = ops[i];
+      }
+      OpRef l, r; double sl, sr;
+      int rc = name_block_ops(BL, po[0], np[0], l, sl);
+      if (rc == 1) return;
+      if (rc != 0) { *err = 1; return; }
+      rc = name_block_ops(BR, po[3], np[3], r, sr);
+      if (rc == 1) return;
+      if (rc != 0) { *err = 1; return; }
+      const int o1 = site_product(ctx->site_ops, po[1], np[1]);
+      const int o2 = site_product(ctx->site_ops, po[2], np[2]);
+      const double c = coef * sl * sr * ((inv & 1) ? -1.0 : 1.0);
+      if (o1 < 0 || o2 < 0 || c == 0.0) return;
+      m[pack_key4(l, o1, o2, r)] += c;
+    };
+    auto add_ops = [&](const EOp* ops, int n, double coef) {
       int err = 0;
-      for (int i = b; i < L; i += NB)
-        for (int j = 0; j < L; ++j) for (int kk = 0; kk < L; ++kk) for (int l = 0; l < L; ++l) {
-          int cnt[4] = {0, 0, 0, 0};
-          ++cnt[part_of(i)]; ++cnt[part_of(j)]; ++cnt[part_of(kk)]; ++cnt[part_of(l)];
-          if (cnt[0] >= 3 || cnt[3] >= 3) continue;                      // inside H^L/H^R or a+ S + h.c.
-          const double wv = 0.5 * W4(ctx, i, j, kk, l);
-          if (wv == 0.0) continue;
-          for (int s = 0; s < 2; ++s) for (int t = 0; t < 2; ++t) {
-            EOp o[4] = {{true, i, s}, {true, j, t}, {false, l, t}, {false, kk, s}};
-            add_ops_to(loc[b], o, 4, wv, &err);
+      add_ops_to(acc, ops, n, coef, &err);
+      DMRG_REQUIRE(!err, DMRG_ERR_ARG, "internal: unnamed operator string");
+    };
+    const OpRef ID{K_ID, 0, false};
+    add_named(OpRef{K_H, 0, false}, 0, 0, ID, 1.0);
+    add_named(ID, 0, 0, OpRef{K_H, 0, false}, 1.0);
+    for (int s = 0; s < 2; ++s) {
+      double mc[16], ma[16];
+      site_elem(true, s, mc);
+      site_elem(false, s, ma);
+      const int oc_ = ctx->site_ops.intern(mc), oa_ = ctx->site_ops.intern(ma);
+      const int sk = s == 0 ? K_SU : K_SD, ck = s == 0 ? K_CU : K_CD;
+      // x outside L:  a+_x S^L_x = - S^L_x a+_x ,  h.c. = (S^L_x)^T a_x
+      for (int x = o_s1; x < L; ++x) {
+        OpRef S{sk, idx_S(BL, x), false}, St{sk, idx_S(BL, x), true};
+        if (x == o_s1) { add_named(S, oc_, 0, ID, -1.0); add_named(St, oa_, 0, ID, 1.0); }
+        else if (x == o_s2) { add_named(S, 0, oc_, ID, -1.0); add_named(St, 0, oa_, ID, 1.0); }
+        else { add_named(S, 0, 0, OpRef{ck, x - BR.lo, false}, -1.0); add_named(St, 0, 0, OpRef{ck, x - BR.lo, true}, 1.0); }
+      }
+      // x outside R:  a+_x S^R_x ,  h.c. = (S^R_x)^T a_x = - a_x (S^R_x)^T
+      for (int x = 0; x <= o_s2; ++x) {
+        OpRef S{sk, idx_S(BR, x), false}, St{sk, idx_S(BR, x), true};
+        if (x == o_s1) { add_named(ID, oc_, 0, S, 1.0); add_named(ID, oa_, 0, St, -1.0); }
+        else if (x == o_s2) { add_named(ID, 0, oc_, S, 1.0); add_named(ID, 0, oa_, St, -1.0); }
+        else { add_named(OpRef{ck, x - BL.lo, false}, 0, 0, S, 1.0); add_named(OpRef{ck, x - BL.lo, true}, 0, 0, St, -1.0); }
+      }
+    }
+    auto is_block = [&](int p) { return p == 0 || p == 3; };
+    for (int i = 0; i < L; ++i) for (int j = 0; j < L; ++j) {
+      int pi = part_of(i), pj = part_of(j);
+      if (pi == pj && is_block(pi)) continue;                        // inside H^L / H^R
+      double f = 1.0;
+      if (pi != pj) f -= 0.5 * (is_block(pi) ? 1 : 0) + 0.5 * (is_block(pj) ? 1 : 0);   // halves carried by S^L, S^R
+      double tv = f * T2(ctx, i, j);
+      if (tv == 0.0) continue;
+      for (int s = 0; s < 2; ++s) {
+        EOp o[2] = {{true, i, s}, {false, j, s}};
+        add_ops(o, 2, tv);
+      }
+    }
+    pt.lap("one-body + S strings");
+    // The L^4 two-body strings: eight buckets (i mod 8) with private maps, processed in parallel and merged
+    // in bucket order, so the coefficient sums do not depend on the number of threads.
+    {
+      constexpr int NB = 8;
+      std::vector<AccMap> loc(NB);
+      int err_any = 0;
+  #pragma omp parallel for num_threads(NB) schedule(static, 1)
+      for (int b = 0; b < NB; ++b) {
+        int err = 0;
+        for (int i = b; i < L; i += NB)
+          for (int j = 0; j < L; ++j) for (int kk = 0; kk < L; ++kk) for (int l = 0; l < L; ++l) {
+            int cnt[4] = {0, 0, 0, 0};
+            ++cnt[part_of(i)]; ++cnt[part_of(j)]; ++cnt[part_of(kk)]; ++cnt[part_of(l)];
+            if (cnt[0] >= 3 || cnt[3] >= 3) continue;                      // inside H^L/H^R or a+ S + h.c.
+            const double wv = 0.5 * W4(ctx, i, j, kk, l);
+            if (wv == 0.0) continue;
+            for (int s = 0; s < 2; ++s) for (int t = 0; t < 2; ++t) {
+              EOp o[4] = {{true, i, s}, {true, j, t}, {false, l, t}, {false, kk, s}};
+              add_ops_to(loc[b], o, 4, wv, &err);
+            }
           }
+        if (err) {
+  #pragma omp atomic write
+          err_any = 1;
         }
-      if (err) {
-#pragma omp atomic write
-        err_any = 1;
+      }
+      DMRG_REQUIRE(!err_any, DMRG_ERR_ARG, "internal: unnamed operator string");
+      pt.lap("two-body strings (parallel)");
+      // merge: partition p takes the keys with key % NB == p from every bucket map, in bucket order
+      parts.resize(NB);
+  #pragma omp parallel for num_threads(NB) schedule(static, 1)
+      for (int p = 0; p < NB; ++p) {
+        AccMap& out = parts[p];
+        for (auto& kv : acc) if ((int)(kv.first % NB) == p) out[kv.first] += kv.second;   // one-body, S, H strings
+        for (int b = 0; b < NB; ++b)
+          for (auto& kv : loc[b]) if ((int)(kv.first % NB) == p) out[kv.first] += kv.second;
       }
     }
-    DMRG_REQUIRE(!err_any, DMRG_ERR_ARG, "internal: unnamed operator string");
-    pt.lap("two-body strings (parallel)");
-    // merge: partition p takes the keys with key % NB == p from every bucket map, in bucket order
-    parts.resize(NB);
-#pragma omp parallel for num_threads(NB) schedule(static, 1)
-    for (int p = 0; p < NB; ++p) {
-      AccMap& out = parts[p];
-      for (auto& kv : acc) if ((int)(kv.first % NB) == p) out[kv.first] += kv.second;   // one-body, S, H strings
-      for (int b = 0; b < NB; ++b)
-        for (auto& kv : loc[b]) if ((int)(kv.first % NB) == p) out[kv.first] += kv.second;
-    }
-  }
-  pt.lap("merge");
-  // ---- group terms; pre-sum one side into complementary operators where that shortens the list ----
-  struct GKey {
-    int lc, lt, o1, o2, rc, rt;
-    bool operator<(const GKey& o) const { return std::tie(lc, lt, o1, o2, rc, rt) < std::tie(o.lc, o.lt, o.o1, o.o2, o.rc, o.rt); }
-  };
-  std::map<GKey, std::vector<Entry>> groups;   // Entry: a = left index, b = right index
-  {
-    std::unordered_map<uint64_t, std::vector<Entry>*> fast;   // group bits of the key -> its entry list
-    const uint64_t gmask = ~((0xFFFull << 38) | (0xFFFull << 1));
-    for (auto& part : parts)
-      for (auto& kv : part) {
-        if (std::fabs(kv.second) < 1e-300) continue;
-        const uint64_t q = kv.first;
-        std::vector<Entry>*& v = fast[q & gmask];
-        if (!v) {
-          GKey g{(int)(q >> 50) & 63, (int)(q >> 37) & 1, (int)(q >> 28) & 511, (int)(q >> 19) & 511,
-                 (int)(q >> 13) & 63, (int)(q & 1)};
-          v = &groups[g];
+    pt.lap("merge");
+    // ---- group terms; pre-sum one side into complementary operators where that shortens the list ----
+    std::map<GKey, std::vector<Entry>> groups;   // Entry: a = left index, b = right index
+    {
+      std::unordered_map<uint64_t, std::vector<Entry>*> fast;   // group bits of the key -> its entry list
+      const uint64_t gmask = ~((0xFFFull << 38) | (0xFFFull << 1));
+      for (auto& part : parts)
+        for (auto& kv : part) {
+          if (std::fabs(kv.second) < 1e-300) continue;
+          const uint64_t q = kv.first;
+          std::vector<Entry>*& v = fast[q & gmask];
+          if (!v) {
+            GKey g{(int)(q >> 50) & 63, (int)(q >> 37) & 1, (int)(q >> 28) & 511, (int)(q >> 19) & 511,
+                   (int)(q >> 13) & 63, (int)(q & 1)};
+            v = &groups[g];
+          }
+          v->push_back(Entry{(int)(q >> 38) & 4095, (int)(q >> 1) & 4095, kv.second});
         }
-        v->push_back(Entry{(int)(q >> 38) & 4095, (int)(q >> 1) & 4095, kv.second});
-      }
-    // a fixed entry order inside every group (the partition maps iterate in hash order)
-    for (auto& kv : groups)
-      std::sort(kv.second.begin(), kv.second.end(), [](const Entry& x, const Entry& y) { return x.a != y.a ? x.a < y.a : x.b < y.b; });
+      // a fixed entry order inside every group (the partition maps iterate in hash order)
+      for (auto& kv : groups)
+        std::sort(kv.second.begin(), kv.second.end(), [](const Entry& x, const Entry& y) { return x.a != y.a ? x.a < y.a : x.b < y.b; });
+    }
+    parts.clear();
+    acc.clear();
+    tg = std::make_shared<TermGroups>();
+    tg->groups = std::move(groups);
+    size_t cached = 0;
+    for (auto& kv : ctx->term_cache) cached += std::static_pointer_cast<TermGroups>(kv.second)->bytes();
+    if (cached + tg->bytes() <= (size_t)1 << 30) ctx->term_cache[k] = tg;   // host memory cap: 1 GiB
+  } else {
+    pt.lap("term groups from cache");
   }
-  parts.clear();
-  acc.clear();
+  const auto& groups = tg->groups;
   Presummer pre(ctx, st);
   struct FG { GKey g; int lcls, rcls; std::vector<Entry> e; };
   std::vector<FG> fgs;

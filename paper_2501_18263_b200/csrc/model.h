@@ -113,6 +113,7 @@ struct dmrg_ctx {
   // environment cache for sweeps: left_cache[i] = block of sites 1..i, right_cache[i] = block of sites i..L.
   // Entries are dropped when a site tensor or bond they depend on changes; total size is capped.
   std::map<int, std::shared_ptr<dmrg::BlockSide>> left_cache, right_cache;
+  std::map<int, std::shared_ptr<void>> term_cache;   // bond k -> term groups of the two-site problem (engine.cu)
   uint64_t cache_bytes() const {
     uint64_t b = 0;
     for (auto& kv : left_cache) b += kv.second->bytes();
