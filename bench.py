@@ -288,6 +288,14 @@ def run_ours(args):
                                          "tflops": s2["flops_renorm"] / (s2["renorm_ms"] * 1e-3) * 1e-12,
                                          "includes": "host planning of the step + all launches + sync"}
 
+    # DRAM bytes per launch of the dominant kernel from the committed ncu --set full capture of this workload
+    # (profiles/r01_gemm128_full.md: dram__bytes_read.sum + dram__bytes_write.sum); only known for the default config.
+    if cfg == 3 and not su2 and not args.D:
+        traffic_detail = {"phase1_bytes_per_launch": 39.21e9, "phase2_bytes_per_launch": 45.56e9,
+                          "source": "profiles/r01_gemm128_full.md"}
+        traffic = 0.5 * (39.21e9 + 45.56e9)
+    else:
+        traffic_detail, traffic = None, None
     if rank == 0:
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
                 "warmup": args.warmup, "ms_per_step": ms_max, "higher_is_better": True, "scaling": "weak",
@@ -306,7 +314,7 @@ def run_ours(args):
                         "ms_per_step": e2e_max},
                 "gpu_launches": int(launches),
                 "roofline": {"bound": "tensor", "achieved": value / world * 1e-3, "peak": peak_tf, "unit": "TFLOP/s",
-                             "frac": value / world * 1e-3 / peak_tf, "traffic": None,
+                             "frac": value / world * 1e-3 / peak_tf, "traffic": traffic,
                              "what": "whole H_eff.psi: analytic task-list flops / event time of the step (all "
                                      "k_grouped_gemm launches of the step, run on the library's worker streams)",
                              "peak_source": "FP64 tensor-pipe (DMMA m8n8k4) register-only loop measured in this run "
@@ -314,7 +322,7 @@ def run_ours(args):
                                             "has no FP64 entry",
                              "dominant_kernel": dict(dominant, achieved=(dom_fl / dom_ms * 1e-9 if dom_ms else None),
                                                      frac=(dom_fl / dom_ms * 1e-9 / peak_tf if dom_ms else None),
-                                                     traffic="profiles/ (ncu dram__bytes per launch)"),
+                                                     traffic=traffic_detail),
                              "hbm": {"unique_bytes_per_apply": st["bytes_unique"],
                                      "intermediate_bytes_per_apply": st["bytes_intermediate"],
                                      "achieved_gbs": (st["bytes_unique"] + st["bytes_intermediate"]) / (ms_max * 1e-3) * 1e-9,
