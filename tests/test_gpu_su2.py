@@ -150,3 +150,35 @@ def test_su2_medium_size_against_oracle():
     assert d.psi_size() == orc.psi_size()
     assert _rel(_apply_gpu(d, v), orc.apply(v)) <= REL_L2
     d.close()
+
+
+def test_su2_input_errors_are_reported():
+    from paper_2501_18263_b200.binding import DMRG, DMRGError
+    L, N = 6, 6
+    T, V = _general_integrals(L, 1)
+    with pytest.raises(DMRGError):
+        DMRG(L, 4, 2, su2=True)                       # SU(2) contexts are total-spin-0 only
+    d = DMRG(L, 3, 3, su2=True)
+    d.load_integrals(T, V)
+    mps = inputs.make_mps_su2(L, N, 8, 3, seed=1)
+    d.mps_set_sectors(mps.sectors)
+    with pytest.raises(DMRGError, match="dmrg_mps_set_site_su2"):
+        d.mps_set_site(1, 0, {((0, 0), 0): np.ones((1, 1))})       # U(1) entry point on an SU(2) context
+    # a q_out that is not a spin coupling of q_in with the site multiplet
+    good = mps.left[2]
+    key = next(k for k in good if k[1] == 1)
+    bad = dict(good)
+    blk = bad.pop(key)
+    wrong = next(q for q in mps.sectors[2] if q not in inputs.su2_couplings(key[0], 1) and mps.sectors[2][q] == blk.shape[1])\
+        if any(q not in inputs.su2_couplings(key[0], 1) and mps.sectors[2][q] == blk.shape[1] for q in mps.sectors[2]) else None
+    if wrong is not None:
+        bad[(key[0], 1, wrong)] = blk
+        with pytest.raises(DMRGError, match="coupling"):
+            d.mps_set_site_su2(2, 0, bad)
+    scaled = {k: v * 1.01 for k, v in good.items()}
+    d.mps_set_site_su2(1, 0, mps.left[1])
+    with pytest.raises(DMRGError, match="left-canonical"):
+        d.mps_set_site_su2(2, 0, scaled)
+    with pytest.raises(DMRGError):
+        d.mps_update_bond(0, {(0, 0): 1})             # bonds 0 and L are fixed
+    d.close()
