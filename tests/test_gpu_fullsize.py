@@ -83,3 +83,25 @@ def test_config3_su2_1024_multiplets_properties():
     d = _ctx(3, su2=True)
     _properties(d, 8, 3)
     d.close()
+
+
+def test_config2_full_size_elementwise_parity():
+    """BASELINE.json configs[2] (L = 30, D = 1024) at its full size against the CPU oracle, element by element
+    (about 100 s of oracle time on the GPU box's host cores).  configs[3] is checked the same way by the one-off
+    script tests/midsize_parity.py (hours of oracle time; result quoted in DESIGN.md)."""
+    import torch
+    from oracle import dmrg as odmrg
+    from paper_2501_18263_b200.binding import DMRG
+    c = inputs.CONFIGS[2]
+    T, V, mps = inputs.make_config(2)
+    v = inputs.make_psi0(mps, c["seed"])
+    d = DMRG(mps.L, mps.n_up, mps.n_dn)
+    d.setup(T, V, mps)
+    got = d.heff_apply(torch.from_numpy(v).cuda()).cpu().numpy()
+    dg = d.heff_diag().cpu().numpy()
+    d.close()
+    orc = odmrg.TwoSiteOracle(T, V, mps.n_up, mps.n_dn, mps.k, mps.sectors, mps.left, mps.right, inputs.psi_blocks(mps))
+    orc.build_env()
+    ref = orc.apply(v)
+    assert np.linalg.norm(got - ref) / np.linalg.norm(ref) <= 1e-11
+    assert np.abs(dg - orc.diag()).max() <= 1e-10
