@@ -1,5 +1,5 @@
-// Grouped, batched, segment-accumulating FP64 GEMM on the DMMA pipe (sm_100a), operands staged by TMA
-// bulk copies from a producer warp (gemm.cu).
+// Grouped, batched, segment-accumulating FP64 GEMM on the DMMA pipe (sm_100a), operands staged by
+// cp.async producer warps into an mbarrier-synchronised shared-memory ring (gemm.cu).
 //
 // One launch executes a list of output tiles of ONE tile shape.  Each output matrix C (M x N) is
 //     C (+)= sum_{seg in segs(C)} sum_{r < seg.count} alpha_seg * op(A_seg[r]) * op(B_seg[r])
