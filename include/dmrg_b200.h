@@ -165,6 +165,7 @@ typedef struct {
   double flops_renorm;      /* analytic flops of the last renormalisation step */
   int64_t total_launches;   /* kernels launched by this context so far */
   double renorm_ms;         /* host+device time of the single blocking step of the last dmrg_renormalize */
+  double flops_shared;      /* phase-1 flops per apply saved by sharing O_L.psi intermediates between term groups */
 } dmrg_stats_t;
 int dmrg_stats(dmrg_ctx* ctx, dmrg_stats_t* out);
 

@@ -47,7 +47,7 @@ class Stats(C.Structure):
                 ("bytes_intermediate", C.c_double), ("psi_size", C.c_int64), ("op_bytes_left", C.c_int64),
                 ("op_bytes_right", C.c_int64), ("n_chunks", C.c_int32), ("launches_per_apply", C.c_int32),
                 ("last_build_ms", C.c_double), ("flops_renorm", C.c_double), ("total_launches", C.c_int64),
-                ("renorm_ms", C.c_double)]
+                ("renorm_ms", C.c_double), ("flops_shared", C.c_double)]
 
     def as_dict(self):
         return {f: getattr(self, f) for f, _ in self._fields_}

@@ -598,6 +598,7 @@ static void finish_superblock(dmrg_ctx* ctx, std::vector<std::vector<DiagTask>>&
   s.n_groups = n_groups;
   s.flops_apply = ctx->apply_plan.flops_analytic;
   s.flops_executed = ctx->apply_plan.flops_executed;
+  s.flops_shared = ctx->apply_plan.flops_shared;
   s.bytes_intermediate = ctx->apply_plan.bytes_intermediate;
   s.psi_size = ctx->psi_n;
   s.op_bytes_left = (int64_t)BL.bytes();

@@ -185,23 +185,42 @@ void Planner::add_piece(const Item& it, int b0, int cnt) {
   const int zr = left_first ? it.X.rows : it.Y.rows;
   const int zc = left_first ? it.Y.cols : it.W.cols;
   const long long zsz = (long long)zr * zc;
-  if (chunks_.back().ws_used + zsz * cnt > cap_) chunks_.emplace_back();
-  HChunk& ch = chunks_.back();
-  const long long zoff = ch.ws_used;
-  ch.ws_used += zsz * cnt;
-  ws_max_ = std::max(ws_max_, ch.ws_used);
-  bi_ += 2.0 * 8.0 * zsz * cnt;
-  fe_ += cnt * std::min(pl, pr);
+  bool shared = false;
+  long long zoff_shared = 0;
   // phase 1: Z[b] = X[b] Y[b]  or  Y[b] W[b].  When only one operand varies with b the `cnt` products
   // are ONE GEMM: operators stacked along M (segmented rows of op(A)) or along N (segmented columns of
   // op(B)); the class storage keeps them contiguous per block, so no copy is needed.
   const Mat& A1 = left_first ? it.X : it.Y;
   const Mat& B1 = left_first ? it.Y : it.W;
+  const double p1f = fl(A1.rows, A1.cols, B1.cols);
+  // The same intermediate is needed by every term group that applies the same operator run to the same psi
+  // block (e.g. a+_l psi for the G5, G12 and G13 patterns): inside a chunk it is computed once.
+  const ZKey zkey{A1.p + b0 * A1.stride, B1.p + b0 * B1.stride, A1.stride, B1.stride, A1.ld, B1.ld, A1.rows, A1.cols,
+                  B1.cols, cnt, (A1.tr ? 1 : 0) | (B1.tr ? 2 : 0)};
+  if (share_z_) {
+    auto f = chunks_.back().zmap.find(zkey);
+    if (f != chunks_.back().zmap.end()) {
+      shared = true;
+      zoff_shared = f->second;
+    }
+  }
+  if (!shared && chunks_.back().ws_used + zsz * cnt > cap_) chunks_.emplace_back();
+  HChunk& ch = chunks_.back();
+  const long long zoff = shared ? zoff_shared : ch.ws_used;
   const bool mergeM = cnt > 1 && A1.stride != 0 && B1.stride == 0;
   const bool mergeN = cnt > 1 && A1.stride == 0 && B1.stride != 0;
   const long long zld = mergeN ? (long long)cnt * zc : zc;       // leading dimension of Z
   const long long zstep = mergeN ? zc : zsz;                      // offset of Z[b] relative to Z[0]
-  {
+  if (shared) {
+    fe_ += cnt * (std::min(pl, pr) - p1f);
+    bi_ += 8.0 * zsz * cnt;                                       // read once more in phase 2
+    fshared_ += cnt * p1f;
+  } else {
+    ch.ws_used += zsz * cnt;
+    ws_max_ = std::max(ws_max_, ch.ws_used);
+    bi_ += 2.0 * 8.0 * zsz * cnt;
+    fe_ += cnt * std::min(pl, pr);
+    if (share_z_) ch.zmap.emplace(zkey, zoff);
     HOut z{};
     z.o.C = reinterpret_cast<double*>(zoff); z.c_ws = true;
     z.o.bsC = zsz; z.o.M = mergeM ? cnt * zr : zr; z.o.N = mergeN ? cnt * zc : zc; z.o.ldc = (int)zld;
@@ -243,6 +262,7 @@ void Planner::finish(Plan* plan, cudaStream_t st) {
   plan->flops_analytic = fa_;
   plan->flops_executed = fe_;
   plan->bytes_intermediate = bi_;
+  plan->flops_shared = fshared_;
   plan->n_items = n_items_;
   plan->n_products = n_products_;
   const bool two_halves = chunks_.size() > 1;

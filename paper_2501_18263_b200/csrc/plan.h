@@ -8,6 +8,7 @@
 // terms stays in registers (no global atomics).  Chunks bound the workspace; outputs accumulate
 // across chunks (they are zeroed by the caller before the plan runs).
 #pragma once
+#include <cstdlib>
 #include <map>
 #include <tuple>
 
@@ -75,6 +76,7 @@ struct Plan {
   bool print_stats = false;   // DMRG_B200_PLAN_STATS: per-shape tile fill printed when a plan is built
   long long ws_half = 0;   // elements per workspace half (two halves when there are several chunks)
   double flops_analytic = 0, flops_executed = 0, bytes_intermediate = 0;
+  double flops_shared = 0;   // phase-1 flops saved by sharing intermediates between term groups
   int64_t n_items = 0, n_products = 0;
   int launches() const;
   // Stages: P1(0) | P2(c-1) + P1(c) ... | P2(last); the launches of a stage are independent (phase 1 of
@@ -97,7 +99,10 @@ class Planner {
  private:
   struct HSeg { GSeg s; bool a_ws, b_ws; };          // *_ws: pointer is a workspace offset
   struct HOut { GOut o; bool c_ws; std::vector<HSeg> segs; int batch; double work; bool c_sc = false; };
+  // identity of a phase-1 product (operands, shapes, batch): equal keys give the same intermediate
+  using ZKey = std::tuple<const double*, const double*, long long, long long, int, int, int, int, int, int, int>;
   struct HChunk {
+    std::map<ZKey, long long> zmap;     // intermediates already in this chunk's workspace
     std::vector<HOut> p1;
     std::vector<HOut> p2;
     std::map<std::tuple<const double*, int, long long>, int> p2_index;  // (C, batch, strideC) -> p2 slot
@@ -109,7 +114,8 @@ class Planner {
   long long cap_;
   std::vector<HChunk> chunks_;
   long long ws_max_ = 0;
-  double fa_ = 0, fe_ = 0, bi_ = 0;
+  double fa_ = 0, fe_ = 0, bi_ = 0, fshared_ = 0;
+  bool share_z_ = std::getenv("DMRG_B200_NO_ZSHARE") == nullptr;
   int64_t n_items_ = 0, n_products_ = 0;
 };
 
