@@ -849,15 +849,20 @@ void prepare_superblock(dmrg_ctx* ctx, cudaStream_t st) {
   Planner planner(&ctx->al, cap);
   std::vector<std::vector<DiagTask>> dtasks(ctx->psi.size());
   int64_t n_tasks = 0, n_groups = 0;
-  for (auto& f : fgs) {
-    const OpClass& CL = *BL.cls[f.lcls];
-    const OpClass& CR = *BR.cls[f.rcls];
-    const auto& m1 = ctx->site_ops.mats[f.g.o1];
-    const auto& m2 = ctx->site_ops.mats[f.g.o2];
-    const int p1 = ctx->site_ops.parity(f.g.o1), p2 = ctx->site_ops.parity(f.g.o2);
-    const int pR = (CR.du + CR.dd) & 1;
-    auto runs = make_runs(f.e);
-    for (size_t bi = 0; bi < ctx->psi.size(); ++bi) {
+  // psi blocks outermost: the items that apply the same operator run to the same psi block (different term
+  // groups) are then neighbours and land in the same workspace chunk, where they share the intermediate
+  std::vector<std::vector<Run>> all_runs;
+  for (auto& f : fgs) all_runs.push_back(make_runs(f.e));
+  for (size_t bi = 0; bi < ctx->psi.size(); ++bi) {
+    for (size_t gi = 0; gi < fgs.size(); ++gi) {
+      const auto& f = fgs[gi];
+      const OpClass& CL = *BL.cls[f.lcls];
+      const OpClass& CR = *BR.cls[f.rcls];
+      const auto& m1 = ctx->site_ops.mats[f.g.o1];
+      const auto& m2 = ctx->site_ops.mats[f.g.o2];
+      const int p1 = ctx->site_ops.parity(f.g.o1), p2 = ctx->site_ops.parity(f.g.o2);
+      const int pR = (CR.du + CR.dd) & 1;
+      const auto& runs = all_runs[gi];
       const PsiBlk& in = ctx->psi[bi];
       // left operator block acting on sector in.qL
       int lb = -1, qLo = in.qL;
