@@ -136,6 +136,24 @@ int dmrg_psi_layout(dmrg_ctx* ctx, int32_t* nblocks, dmrg_psi_block* h_blocks, i
 /* psi_out = H_eff psi_in (Eq. (7)/(8)); e_core is included.  Overwrites d_psi_out. */
 int dmrg_heff_apply(dmrg_ctx* ctx, const double* d_psi_in, double* d_psi_out, void* stream);
 
+/* Sharding of H_eff.psi over `count` ranks, one process per GPU (the tasks are "independent operations";
+ * PAPER.md:25 multi-GPU).  Call before dmrg_env_build / dmrg_renormalize.  Every rank holds the whole MPS and both
+ * environments and prepares the same two-site problem; the psi' blocks are dealt to the ranks by analytic flops
+ * (largest first to the least loaded rank — the same map on every rank), and rank r keeps only the tasks whose
+ * OUTPUT block it owns.  A psi' block is therefore computed completely by one rank and is exactly zero on the
+ * others, so the exchange is a plain sum.  With `reduce` set, dmrg_heff_apply and dmrg_davidson call
+ * reduce(user, d_buf, n, stream) after the local tasks of every apply; it must replace the n doubles at the device
+ * pointer d_buf by their sum over all ranks, enqueued on `stream` (the binding uses torch.distributed.all_reduce over
+ * NCCL), and return 0.  With reduce = NULL dmrg_heff_apply returns the rank's partial result (e_core.psi is added
+ * by rank 0 only) and the caller sums; dmrg_davidson then fails with DMRG_ERR_ARG.  diag(H_eff) is whole on every
+ * rank.  count = 1 restores the unsharded library. */
+typedef int (*dmrg_reduce_fn)(void* user, double* d_buf, int64_t n, void* stream);
+int dmrg_set_shard(dmrg_ctx* ctx, int32_t rank, int32_t count, dmrg_reduce_fn reduce, void* user);
+
+/* Owner rank of every psi block (h_owner: nblocks ints) and the analytic flops per rank (h_flops: `count` doubles)
+ * of the prepared problem; either pointer may be NULL. */
+int dmrg_shard_info(dmrg_ctx* ctx, int32_t* h_owner, double* h_flops);
+
 /* Diagonal of H_eff in the psi layout. */
 int dmrg_heff_diag(dmrg_ctx* ctx, double* d_diag, void* stream);
 

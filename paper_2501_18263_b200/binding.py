@@ -22,9 +22,10 @@ EXPORTS = [
     "dmrg_mps_set_site", "dmrg_env_build", "dmrg_renormalize", "dmrg_psi_layout", "dmrg_heff_apply",
     "dmrg_heff_diag", "dmrg_davidson", "dmrg_heff_apply_host", "dmrg_davidson_host", "dmrg_stats",
     "dmrg_env_export", "dmrg_fp64_peak", "dmrg_apply_profile", "dmrg_mps_set_site_su2", "dmrg_su2_f_factor",
-    "dmrg_mps_update_bond",
+    "dmrg_mps_update_bond", "dmrg_set_shard", "dmrg_shard_info",
 ]
 
+REDUCE_FN = C.CFUNCTYPE(C.c_int, C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p)
 ALLOC_FN = C.CFUNCTYPE(C.c_void_p, C.c_uint64, C.c_void_p)
 FREE_FN = C.CFUNCTYPE(None, C.c_void_p, C.c_void_p)
 
@@ -87,6 +88,8 @@ def load_library(build_if_missing: bool = True):
     lib.dmrg_psi_layout.argtypes = [vp, C.POINTER(i32), C.POINTER(PsiBlock), C.POINTER(i64)]
     lib.dmrg_heff_apply.argtypes = [vp, vp, vp, vp]
     lib.dmrg_heff_diag.argtypes = [vp, vp, vp]
+    lib.dmrg_set_shard.argtypes = [vp, i32, i32, REDUCE_FN, vp]
+    lib.dmrg_shard_info.argtypes = [vp, vp, vp]
     lib.dmrg_davidson.argtypes = [vp, vp, C.c_double, i32, i32, dp, C.POINTER(i32), dp, vp]
     lib.dmrg_heff_apply_host.argtypes = [vp, vp, vp, vp]
     lib.dmrg_davidson_host.argtypes = [vp, vp, C.c_double, i32, i32, dp, C.POINTER(i32), dp, vp]
@@ -223,6 +226,36 @@ class DMRG:
 
     def renormalize(self, direction):
         self._check(self.lib.dmrg_renormalize(self.ctx, direction, self._stream()))
+
+    def set_shard(self, rank, count, reduce=None):
+        """dmrg_set_shard.  `reduce(t)` must sum the float64 device tensor `t` over all ranks in place (e.g.
+        `lambda t: torch.distributed.all_reduce(t)`); None = partial results, the caller sums."""
+        if reduce is None or count <= 1:
+            self._reduce_cb = REDUCE_FN(0)
+        else:
+            torch = self.torch
+
+            def _cb(_user, ptr, n, _stream):
+                try:
+                    buf = self._live[ptr]     # the library's padded psi' buffer, allocated through _alloc
+                    reduce(buf.view(torch.float64)[:n])
+                    return 0
+                except Exception:             # no exception may cross the C boundary
+                    import traceback
+                    traceback.print_exc()
+                    return 1
+
+            self._reduce_cb = REDUCE_FN(_cb)
+        self._check(self.lib.dmrg_set_shard(self.ctx, int(rank), int(count), self._reduce_cb, None))
+        self.shard = (int(rank), int(count))
+
+    def shard_info(self):
+        """(owner rank per psi block, analytic flops per rank) of the prepared problem."""
+        nb = len(self.psi_layout()[0])
+        owner = np.zeros(nb, dtype=np.int32)
+        flops = np.zeros(getattr(self, "shard", (0, 1))[1], dtype=np.float64)
+        self._check(self.lib.dmrg_shard_info(self.ctx, _np_ptr(owner), _np_ptr(flops)))
+        return owner, flops
 
     def psi_layout(self):
         nb, n = C.c_int32(), C.c_int64()

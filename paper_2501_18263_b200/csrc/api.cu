@@ -356,11 +356,23 @@ int dmrg_psi_layout(dmrg_ctx* ctx, int32_t* nblocks, dmrg_psi_block* out, int64_
   API_END
 }
 
+// sharded contexts: sum of the ranks' disjoint psi' blocks (padded layout), through the caller's collective
+static void shard_reduce(dmrg_ctx* ctx, cudaStream_t st) {
+  if (ctx->shard_count <= 1 || !ctx->reduce_cb) return;
+  const int rc = ctx->reduce_cb(ctx->reduce_user, ctx->psi_out_p.p, (int64_t)ctx->psi_np, (void*)st);
+  DMRG_REQUIRE(rc == 0, DMRG_ERR_ARG, "heff_apply: the reduce callback of dmrg_set_shard failed");
+}
+// e_core.psi is added once: by every rank after a reduce, by rank 0 alone when the caller sums partial results
+static double shard_e_core(const dmrg_ctx* ctx) {
+  return (ctx->shard_count > 1 && !ctx->reduce_cb && ctx->shard_rank != 0) ? 0.0 : ctx->e_core;
+}
+
 // psi_out_p = H_eff psi_in_p on the padded internal buffers
 static void apply_padded(dmrg_ctx* ctx, cudaStream_t st) {
   DMRG_CUDA(cudaMemsetAsync(ctx->psi_out_p.p, 0, (size_t)ctx->psi_np * 8, st));
   ++ctx->launches;
   ctx->apply_plan.run(st, &ctx->launches, ctx->ex());
+  shard_reduce(ctx, st);
 }
 
 int dmrg_heff_apply(dmrg_ctx* ctx, const double* d_in, double* d_out, void* stream) {
@@ -369,7 +381,7 @@ int dmrg_heff_apply(dmrg_ctx* ctx, const double* d_in, double* d_out, void* stre
   DMRG_REQUIRE(ctx->k > 0 && d_in && d_out, DMRG_ERR_ARG, "heff_apply: no problem prepared or null pointer");
   launch_pack(ctx->d_psi_blocks.p, (int)ctx->psi.size(), d_in, ctx->psi_in_p.p, st);
   apply_padded(ctx, st);
-  launch_unpack(ctx->d_psi_blocks.p, (int)ctx->psi.size(), ctx->psi_out_p.p, d_out, ctx->e_core, d_in, st);
+  launch_unpack(ctx->d_psi_blocks.p, (int)ctx->psi.size(), ctx->psi_out_p.p, d_out, shard_e_core(ctx), d_in, st);
   ctx->launches += 2;
   DMRG_CUDA(cudaGetLastError());
   API_END
@@ -518,6 +530,7 @@ int dmrg_davidson(dmrg_ctx* ctx, double* d_psi, double tol, int32_t max_iter, in
   API_BEGIN
   cudaStream_t st = (cudaStream_t)stream;
   DMRG_REQUIRE(ctx->k > 0 && d_psi && h_energy && h_iters && h_resid, DMRG_ERR_ARG, "davidson: bad arguments");
+  DMRG_REQUIRE(ctx->shard_count <= 1 || ctx->reduce_cb, DMRG_ERR_ARG, "davidson: a sharded context needs the reduce callback");
   DevArray<double> xp;
   xp.allocate(&ctx->al, (size_t)ctx->psi_np);
   DMRG_CUDA(cudaMemsetAsync(xp.p, 0, (size_t)ctx->psi_np * 8, st));
@@ -557,6 +570,27 @@ int dmrg_davidson_host(dmrg_ctx* ctx, double* h_psi, double tol, int32_t max_ite
   if (rc != DMRG_OK) return rc;
   DMRG_CUDA(cudaMemcpyAsync(h_psi, a.p, (size_t)ctx->psi_n * 8, cudaMemcpyDeviceToHost, st));
   DMRG_CUDA(cudaStreamSynchronize(st));
+  API_END
+}
+
+int dmrg_set_shard(dmrg_ctx* ctx, int32_t rank, int32_t count, dmrg_reduce_fn reduce, void* user) {
+  API_BEGIN
+  DMRG_REQUIRE(count >= 1 && rank >= 0 && rank < count, DMRG_ERR_ARG, "set_shard: need 0 <= rank < count");
+  ctx->shard_rank = rank;
+  ctx->shard_count = count;
+  ctx->reduce_cb = count > 1 ? reduce : nullptr;
+  ctx->reduce_user = user;
+  // a prepared problem belongs to the old sharding
+  ctx->k = 0;
+  ctx->apply_plan.clear();
+  API_END
+}
+
+int dmrg_shard_info(dmrg_ctx* ctx, int32_t* h_owner, double* h_flops) {
+  API_BEGIN
+  DMRG_REQUIRE(ctx->k > 0, DMRG_ERR_ARG, "shard_info: no problem prepared");
+  if (h_owner) for (size_t i = 0; i < ctx->psi.size(); ++i) h_owner[i] = ctx->psi_owner[i];
+  if (h_flops) for (int r = 0; r < ctx->shard_count; ++r) h_flops[r] = r < (int)ctx->shard_flops.size() ? ctx->shard_flops[r] : 0.0;
   API_END
 }
 
@@ -618,7 +652,8 @@ int dmrg_apply_profile(dmrg_ctx* ctx, const double* d_in, double* d_out, int32_t
   DMRG_CUDA(cudaMemsetAsync(ctx->psi_out_p.p, 0, (size_t)ctx->psi_np * 8, st));
   std::vector<LaunchRecord> rec;
   ctx->apply_plan.run_profiled(st, &rec);
-  launch_unpack(ctx->d_psi_blocks.p, (int)ctx->psi.size(), ctx->psi_out_p.p, d_out, ctx->e_core, d_in, st);
+  shard_reduce(ctx, st);
+  launch_unpack(ctx->d_psi_blocks.p, (int)ctx->psi.size(), ctx->psi_out_p.p, d_out, shard_e_core(ctx), d_in, st);
   ctx->launches += 3 + (int64_t)rec.size();
   DMRG_CUDA(cudaStreamSynchronize(st));
   *n = (int32_t)rec.size();

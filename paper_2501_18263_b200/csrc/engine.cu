@@ -566,6 +566,25 @@ struct TermGroups {
   size_t bytes() const { size_t b = 0; for (auto& kv : groups) b += kv.second.size() * sizeof(Entry); return b; }
 };
 
+// Output-block sharding of H_eff.psi over ranks ("independent operations"): every psi'
+// block is computed completely by one rank, so the exchange is a sum with exact zeros.  Longest-processing-time
+// assignment on the analytic flops per output block; ties by block index and rank, so all ranks agree.
+static void assign_shard_owners(dmrg_ctx* ctx, const std::vector<double>& blk_flops) {
+  const size_t nb = ctx->psi.size();
+  ctx->psi_owner.assign(nb, 0);
+  ctx->shard_flops.assign((size_t)std::max(1, ctx->shard_count), 0.0);
+  if (ctx->shard_count <= 1) return;
+  std::vector<int> order(nb);
+  for (size_t i = 0; i < nb; ++i) order[i] = (int)i;
+  std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return blk_flops[a] > blk_flops[b]; });
+  for (int b : order) {
+    int best = 0;
+    for (int r = 1; r < ctx->shard_count; ++r) if (ctx->shard_flops[r] < ctx->shard_flops[best]) best = r;
+    ctx->psi_owner[b] = best;
+    ctx->shard_flops[best] += blk_flops[b];
+  }
+}
+
 // diag(H_eff) from the diagonal tasks, and the statistics of the prepared two-site problem
 static void finish_superblock(dmrg_ctx* ctx, std::vector<std::vector<DiagTask>>& dtasks, int64_t n_terms,
                               int64_t n_tasks, int64_t n_groups, cudaStream_t st) {
@@ -853,6 +872,11 @@ void prepare_superblock(dmrg_ctx* ctx, cudaStream_t st) {
   // groups) are then neighbours and land in the same workspace chunk, where they share the intermediate
   std::vector<std::vector<Run>> all_runs;
   for (auto& f : fgs) all_runs.push_back(make_runs(f.e));
+  // Sharded contexts (dmrg_set_shard) run the loop twice: pass 0 only adds up the analytic flops per OUTPUT block,
+  // from which every rank derives the same block -> rank map; pass 1 emits the items of the blocks this rank owns.
+  std::vector<double> blk_flops(ctx->psi.size(), 0.0);
+  for (int pass = ctx->shard_count > 1 ? 0 : 1; pass < 2; ++pass) {
+  if (pass == 1) assign_shard_owners(ctx, blk_flops);
   for (size_t bi = 0; bi < ctx->psi.size(); ++bi) {
     for (size_t gi = 0; gi < fgs.size(); ++gi) {
       const auto& f = fgs[gi];
@@ -892,9 +916,10 @@ void prepare_superblock(dmrg_ctx* ctx, cudaStream_t st) {
           int n1 = SITE_QU[in.s1] + SITE_QD[in.s1], n2 = SITE_QU[in.s2] + SITE_QD[in.s2];
           int ph = nL * (p1 + p2 + pR) + n1 * (p2 + pR) + n2 * pR;
           const double sgn = (ph & 1) ? -1.0 : 1.0;
-          ++n_groups;
+          const bool mine = ctx->psi_owner[fo->second] == ctx->shard_rank;
+          if (pass == 1 && mine) ++n_groups;
           for (auto& r : runs) {
-            n_tasks += r.cnt;
+            if (pass == 1 && mine) n_tasks += r.cnt;
             Item it;
             it.C = ctx->psi_out_p.p + out.off_p; it.ldc = out.dRp; it.strideC = 0;
             it.count = r.cnt; it.alpha = r.c * v1 * v2 * sgn;
@@ -917,8 +942,9 @@ void prepare_superblock(dmrg_ctx* ctx, cudaStream_t st) {
               it.nmat = 2; it.X = Xp;
               it.Y = Mat{I.ptr(ib, 0), I.blocks[ib].cp, false, 0, in.dRp, in.dRp, in.dR, in.dR};
             }
-            planner.add(it);
-            if (fo->second == (int)bi) {
+            if (pass == 0) { blk_flops[fo->second] += item_flops(it); continue; }
+            if (mine) planner.add(it);
+            if (fo->second == (int)bi) {      // the diagonal is kept whole on every rank
               DiagTask d{};
               d.L = lb >= 0 ? CL.ptr(lb, r.a0) : nullptr;
               d.R = rb >= 0 ? CR.ptr(rb, r.b0) : nullptr;
@@ -934,6 +960,7 @@ void prepare_superblock(dmrg_ctx* ctx, cudaStream_t st) {
         }
       }
     }
+  }
   }
   pt.lap("tasks -> items");
   planner.finish(&ctx->apply_plan, st);

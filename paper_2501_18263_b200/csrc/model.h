@@ -134,6 +134,12 @@ struct dmrg_ctx {
   dmrg::DevArray<dmrg::PsiBlockDev> d_psi_blocks;
   dmrg::DevArray<double> psi_in_p, psi_out_p, diag_p;
   dmrg::Plan apply_plan;
+  // output-block sharding of the apply over ranks (dmrg_set_shard); psi_owner[block] = rank that computes it
+  int shard_rank = 0, shard_count = 1;
+  dmrg_reduce_fn reduce_cb = nullptr;
+  void* reduce_user = nullptr;
+  std::vector<int> psi_owner;
+  std::vector<double> shard_flops;               // analytic flops per rank of the prepared problem
   dmrg::Exec exec;                              // worker streams (plan.h)
   dmrg::Exec* ex() { return exec.ok ? &exec : nullptr; }
   dmrg_stats_t stats{};

@@ -125,14 +125,12 @@ void Planner::add(const Item& it) {
   ++n_items_;
   n_products_ += it.count;
   if (it.nmat == 2) {
-    fa_ += it.count * fl(it.X.urows, it.X.ucols, it.Y.ucols);
+    fa_ += item_flops(it);
     add_piece(it, 0, it.count);
     return;
   }
   // analytic flops: the cheaper order on the true (unpadded) dims
-  double left = fl(it.X.urows, it.X.ucols, it.Y.ucols) + fl(it.X.urows, it.Y.ucols, it.W.ucols);
-  double right = fl(it.Y.urows, it.Y.ucols, it.W.ucols) + fl(it.X.urows, it.X.ucols, it.W.ucols);
-  fa_ += it.count * std::min(left, right);
+  fa_ += item_flops(it);
   // workspace per product, in the order the kernels will use (padded dims)
   double pl = fl(it.X.rows, it.X.cols, it.Y.cols) + fl(it.X.rows, it.Y.cols, it.W.cols);
   double pr = fl(it.Y.rows, it.Y.cols, it.W.cols) + fl(it.X.rows, it.X.cols, it.W.cols);

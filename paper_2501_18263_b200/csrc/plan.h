@@ -39,6 +39,15 @@ struct Item {
   Mat X, Y, W;
 };
 
+// analytic flops of an item: the cheaper contraction order on the true (unpadded) dims
+inline double item_flops(const Item& it) {
+  auto fl = [](double m, double k, double n) { return 2.0 * m * k * n; };
+  if (it.nmat == 2) return it.count * fl(it.X.urows, it.X.ucols, it.Y.ucols);
+  const double left = fl(it.X.urows, it.X.ucols, it.Y.ucols) + fl(it.X.urows, it.Y.ucols, it.W.ucols);
+  const double right = fl(it.Y.urows, it.Y.ucols, it.W.ucols) + fl(it.X.urows, it.X.ucols, it.W.ucols);
+  return it.count * std::min(left, right);
+}
+
 struct Phase {
   DevArray<GOut> outs;
   DevArray<GSeg> segs;
