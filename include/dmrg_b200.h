@@ -64,6 +64,9 @@ typedef struct {
   dmrg_alloc_fn alloc;
   dmrg_free_fn free;
   void* alloc_user;
+  uint64_t env_host_bytes;  /* host tier of the environment cache: cached blocks that no longer fit the device cap are
+                               moved to pinned host memory (up to this many bytes) instead of being dropped, and copied
+                               back when a sweep needs them; 0 = no host tier */
 } dmrg_config;
 
 int dmrg_create(const dmrg_config* cfg, dmrg_ctx** out);
@@ -184,6 +187,9 @@ typedef struct {
   int64_t total_launches;   /* kernels launched by this context so far */
   double renorm_ms;         /* host+device time of the single blocking step of the last dmrg_renormalize */
   double flops_shared;      /* phase-1 flops per apply saved by sharing O_L.psi intermediates between term groups */
+  int64_t env_spills, env_fetches;   /* environment blocks moved to / back from the host tier so far */
+  double env_host_bytes;    /* pinned host memory held by the host tier */
+  double env_device_bytes;  /* device-resident bytes of the cached environment blocks */
 } dmrg_stats_t;
 int dmrg_stats(dmrg_ctx* ctx, dmrg_stats_t* out);
 

@@ -33,7 +33,7 @@ FREE_FN = C.CFUNCTYPE(None, C.c_void_p, C.c_void_p)
 class Config(C.Structure):
     _fields_ = [("L", C.c_int32), ("n_up", C.c_int32), ("n_dn", C.c_int32), ("symmetry", C.c_int32),
                 ("device", C.c_int32), ("workspace_bytes", C.c_uint64), ("env_cache_bytes", C.c_uint64), ("alloc", ALLOC_FN),
-                ("free", FREE_FN), ("alloc_user", C.c_void_p)]
+                ("free", FREE_FN), ("alloc_user", C.c_void_p), ("env_host_bytes", C.c_uint64)]
 
 
 class PsiBlock(C.Structure):
@@ -48,7 +48,8 @@ class Stats(C.Structure):
                 ("bytes_intermediate", C.c_double), ("psi_size", C.c_int64), ("op_bytes_left", C.c_int64),
                 ("op_bytes_right", C.c_int64), ("n_chunks", C.c_int32), ("launches_per_apply", C.c_int32),
                 ("last_build_ms", C.c_double), ("flops_renorm", C.c_double), ("total_launches", C.c_int64),
-                ("renorm_ms", C.c_double), ("flops_shared", C.c_double)]
+                ("renorm_ms", C.c_double), ("flops_shared", C.c_double), ("env_spills", C.c_int64),
+                ("env_fetches", C.c_int64), ("env_host_bytes", C.c_double), ("env_device_bytes", C.c_double)]
 
     def as_dict(self):
         return {f: getattr(self, f) for f, _ in self._fields_}
@@ -115,7 +116,7 @@ def _np_ptr(a):
 class DMRG:
     """One library context on one GPU.  Methods carry the names of the C calls (without `dmrg_`)."""
 
-    def __init__(self, L, n_up, n_dn, device=0, workspace_bytes=0, su2=False, env_cache_bytes=0):
+    def __init__(self, L, n_up, n_dn, device=0, workspace_bytes=0, su2=False, env_cache_bytes=0, env_host_bytes=0):
         import torch
         if not torch.cuda.is_available():
             raise DMRGError("CUDA device required: the library has no CPU path")
@@ -139,7 +140,7 @@ class DMRG:
         self._free_cb = FREE_FN(_free)
         self.su2 = bool(su2)
         self.cfg = Config(L, n_up, n_dn, 1 if su2 else 0, device, workspace_bytes, env_cache_bytes, self._alloc_cb,
-                          self._free_cb, None)
+                          self._free_cb, None, env_host_bytes)
         self.ctx = C.c_void_p()
         rc = self.lib.dmrg_create(C.byref(self.cfg), C.byref(self.ctx))
         if rc != 0:

@@ -26,6 +26,35 @@ using namespace dmrg;
     return DMRG_ERR_ARG;                           \
   }
 
+namespace dmrg {
+double* HostPool::get(uint64_t bytes, uint64_t* got) {
+  // size classes, so that buffers get re-used: powers of two from 64 KiB, multiples of 256 MiB above that
+  if (bytes > (1ull << 28)) bytes = (bytes + ((1ull << 28) - 1)) & ~((1ull << 28) - 1);
+  else { uint64_t c = 1ull << 16; while (c < bytes) c <<= 1; bytes = c; }
+  int best = -1;
+  for (int i = 0; i < (int)free_list.size(); ++i)
+    if (free_list[i].second >= bytes && (best < 0 || free_list[i].second < free_list[best].second)) best = i;
+  if (best >= 0) {
+    auto pr = free_list[best];
+    free_list.erase(free_list.begin() + best);
+    *got = pr.second;
+    return pr.first;
+  }
+  while (total + bytes > cap && !free_list.empty()) {             // make room from buffers that are too small
+    cudaFreeHost(free_list.back().first);
+    total -= free_list.back().second;
+    free_list.pop_back();
+  }
+  if (total + bytes > cap) return nullptr;
+  void* p = nullptr;
+  if (cudaMallocHost(&p, bytes) != cudaSuccess) { cudaGetLastError(); return nullptr; }
+  total += bytes;
+  *got = bytes;
+  return static_cast<double*>(p);
+}
+HostPool::~HostPool() { for (auto& f : free_list) cudaFreeHost(f.first); }
+}  // namespace dmrg
+
 extern "C" {
 
 int dmrg_create(const dmrg_config* cfg, dmrg_ctx** out) {
@@ -48,6 +77,10 @@ int dmrg_create(const dmrg_config* cfg, dmrg_ctx** out) {
   c->L = cfg->L;
   c->site.resize(cfg->L + 2);
   c->site_ops.build_products();
+  if (cfg->env_host_bytes) {
+    c->host_pool = std::make_shared<dmrg::HostPool>();
+    c->host_pool->cap = cfg->env_host_bytes;
+  }
   try {
     if (!std::getenv("DMRG_B200_SERIAL")) c->exec.init();   // debugging aid: every launch in order on one stream
   } catch (const dmrg::Error&) {
@@ -251,9 +284,73 @@ static uint64_t env_cache_cap(const dmrg_ctx* ctx) {
   return tot / 8;
 }
 
-static void cache_put(dmrg_ctx* ctx, bool left, int key, const std::shared_ptr<BlockSide>& b) {
-  if (ctx->cache_bytes() + b->bytes() > env_cache_cap(ctx)) return;
+// ---- host tier of the environment cache (cfg.env_host_bytes) ----
+static bool spill_block(dmrg_ctx* ctx, BlockSide& b, cudaStream_t st) {
+  if (b.spilled) return true;
+  if (!ctx->host_pool) return false;
+  uint64_t bytes = 0;
+  for (auto& c : b.cls) if (c && c->data.p) bytes += (uint64_t)c->data.n * 8;
+  uint64_t got = 0;
+  double* h = ctx->host_pool->get(std::max<uint64_t>(bytes, 8), &got);
+  if (!h) return false;
+  b.host_n.assign(b.cls.size(), 0);
+  uint64_t off = 0;
+  for (size_t i = 0; i < b.cls.size(); ++i) {
+    OpClass* c = b.cls[i].get();
+    if (!c || !c->data.p) continue;
+    DMRG_CUDA(cudaMemcpyAsync(h + off, c->data.p, c->data.n * 8, cudaMemcpyDeviceToHost, st));
+    b.host_n[i] = c->data.n;
+    off += c->data.n;
+  }
+  DMRG_CUDA(cudaStreamSynchronize(st));
+  for (auto& c : b.cls) if (c) c->data.release();
+  b.host = h; b.host_bytes = got; b.pool = ctx->host_pool; b.spilled = true;
+  ++ctx->n_spills;
+  return true;
+}
+
+static void fetch_block(dmrg_ctx* ctx, BlockSide& b, cudaStream_t st) {
+  if (!b.spilled) return;
+  uint64_t off = 0;
+  for (size_t i = 0; i < b.cls.size(); ++i) {
+    OpClass* c = b.cls[i].get();
+    if (!c || !b.host_n[i]) continue;
+    c->data.allocate(&ctx->al, b.host_n[i]);
+    DMRG_CUDA(cudaMemcpyAsync(c->data.p, b.host + off, b.host_n[i] * 8, cudaMemcpyHostToDevice, st));
+    off += b.host_n[i];
+  }
+  DMRG_CUDA(cudaStreamSynchronize(st));
+  b.pool->put(b.host, b.host_bytes);
+  b.host = nullptr; b.host_bytes = 0; b.pool.reset(); b.spilled = false;
+  ++ctx->n_fetches;
+}
+
+// Keeps the device-resident part of the cache under its cap: the resident block farthest from bond `near` goes to
+// the host tier, or is dropped when there is none (or it is full).  The blocks in use are never touched.
+static void cache_enforce(dmrg_ctx* ctx, int near, cudaStream_t st) {
+  const uint64_t cap = env_cache_cap(ctx);
+  while (true) {
+    uint64_t res = 0;
+    std::shared_ptr<BlockSide> far;
+    bool far_left = true; int far_key = 0, far_dist = -1;
+    for (int side = 0; side < 2; ++side)
+      for (auto& kv : (side == 0 ? ctx->left_cache : ctx->right_cache)) {
+        if (kv.second->spilled) continue;
+        res += kv.second->bytes();
+        if (kv.second == ctx->left || kv.second == ctx->right) continue;
+        const int dist = std::abs(kv.first - near);
+        if (dist > far_dist) { far_dist = dist; far = kv.second; far_left = side == 0; far_key = kv.first; }
+      }
+    if (res <= cap || !far) return;
+    drop_presummed(*far, ctx->su2());
+    if (!spill_block(ctx, *far, st)) (far_left ? ctx->left_cache : ctx->right_cache).erase(far_key);
+  }
+}
+
+static void cache_put(dmrg_ctx* ctx, bool left, int key, const std::shared_ptr<BlockSide>& b, cudaStream_t st) {
+  if (!ctx->host_pool && ctx->cache_bytes() + b->bytes() > env_cache_cap(ctx)) return;   // no host tier: first come
   (left ? ctx->left_cache : ctx->right_cache)[key] = b;
+  if (ctx->host_pool) cache_enforce(ctx, key, st);
 }
 
 static void build_side(dmrg_ctx* ctx, bool left, int upto, cudaStream_t st, double* flops_last) {
@@ -267,10 +364,17 @@ static void build_side(dmrg_ctx* ctx, bool left, int upto, cudaStream_t st, doub
     for (auto& kv : ctx->right_cache) if (kv.first >= upto && kv.first <= from) { from = kv.first; blk = kv.second; }
   }
   if (!blk) blk = su ? su2e::vacuum_block_su2(ctx, left, st) : vacuum_block(ctx, left, st);
+  if (blk->spilled) {
+    // make room first: the block about to come back counts as needed
+    fetch_block(ctx, *blk, st);
+    (left ? ctx->left : ctx->right) = blk;
+    cache_enforce(ctx, upto, st);
+  }
   auto step = [&](int i) {
     std::shared_ptr<BlockSide> nb = su ? renormalize_block_su2(ctx, *blk, i, st, flops_last)
                                        : renormalize_block(ctx, *blk, i, st, flops_last);
-    cache_put(ctx, left, i, nb);
+    (left ? ctx->left : ctx->right) = nb;     // in use: the cache must not move it to the host tier
+    cache_put(ctx, left, i, nb, st);
     return nb;
   };
   if (left) for (int i = from + 1; i <= upto; ++i) blk = step(i);
@@ -285,6 +389,8 @@ int dmrg_env_build(dmrg_ctx* ctx, int32_t k, void* stream) {
   DMRG_REQUIRE(k >= 1 && k + 1 <= ctx->L, DMRG_ERR_ARG, "env_build: bond out of range");
   auto t0 = std::chrono::steady_clock::now();
   ctx->apply_plan.clear();
+  if (ctx->left) drop_presummed(*ctx->left, ctx->su2());      // they may stay in the cache: carried operators only
+  if (ctx->right) drop_presummed(*ctx->right, ctx->su2());
   ctx->left.reset();
   ctx->right.reset();
   double fl = 0;
@@ -305,11 +411,13 @@ int dmrg_renormalize(dmrg_ctx* ctx, int32_t direction, void* stream) {
   const int k = ctx->k;
   double fl = 0;
   ctx->apply_plan.clear();
+  drop_presummed(*ctx->left, ctx->su2());
+  drop_presummed(*ctx->right, ctx->su2());
   if (direction == 0) {
     DMRG_REQUIRE(k + 2 <= ctx->L, DMRG_ERR_ARG, "renormalize: already at the right end");
     auto r0 = std::chrono::steady_clock::now();
     ctx->left = ctx->su2() ? renormalize_block_su2(ctx, *ctx->left, k, st, &fl) : renormalize_block(ctx, *ctx->left, k, st, &fl);
-    cache_put(ctx, true, k, ctx->left);
+    cache_put(ctx, true, k, ctx->left, st);
     ctx->stats.renorm_ms = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - r0).count();
     double f2 = 0;
     ctx->right.reset();
@@ -320,7 +428,7 @@ int dmrg_renormalize(dmrg_ctx* ctx, int32_t direction, void* stream) {
     auto r0 = std::chrono::steady_clock::now();
     ctx->right = ctx->su2() ? renormalize_block_su2(ctx, *ctx->right, k + 1, st, &fl)
                             : renormalize_block(ctx, *ctx->right, k + 1, st, &fl);
-    cache_put(ctx, false, k + 1, ctx->right);
+    cache_put(ctx, false, k + 1, ctx->right, st);
     ctx->stats.renorm_ms = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - r0).count();
     double f2 = 0;
     ctx->left.reset();
@@ -598,6 +706,10 @@ int dmrg_stats(dmrg_ctx* ctx, dmrg_stats_t* out) {
   API_BEGIN
   DMRG_REQUIRE(out, DMRG_ERR_ARG, "stats: null pointer");
   ctx->stats.total_launches = ctx->launches;
+  ctx->stats.env_spills = ctx->n_spills;
+  ctx->stats.env_fetches = ctx->n_fetches;
+  ctx->stats.env_host_bytes = ctx->host_pool ? (double)ctx->host_pool->total : 0.0;
+  ctx->stats.env_device_bytes = (double)ctx->cache_bytes();
   *out = ctx->stats;
   API_END
 }

@@ -971,4 +971,13 @@ void prepare_superblock(dmrg_ctx* ctx, cudaStream_t st) {
 
 #include "engine_su2.inc"
 
+void drop_presummed(BlockSide& b, bool su2) {
+  if (!su2) {
+    if ((int)b.cls.size() > K_NSTD) b.cls.resize(K_NSTD);
+  } else if ((int)b.kinds.size() > su2e::SK_N) {
+    b.cls.resize(b.kinds[su2e::SK_N - 1].cids.back() + 1);
+    b.kinds.resize(su2e::SK_N);
+  }
+}
+
 }  // namespace dmrg

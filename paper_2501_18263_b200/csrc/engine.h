@@ -16,6 +16,9 @@ std::unique_ptr<BlockSide> renormalize_block(dmrg_ctx* ctx, const BlockSide& old
 // Vacuum block left of site 1 / right of site L.
 std::unique_ptr<BlockSide> vacuum_block(dmrg_ctx* ctx, bool is_left, cudaStream_t st);
 
+// Frees the pre-summed (complementary) classes a two-site problem attached to a block; the carried ones stay.
+void drop_presummed(BlockSide& b, bool su2);
+
 // Two-site problem at bond (k, k+1): psi layout, complementary operators, apply plan, diagonal.
 void prepare_superblock(dmrg_ctx* ctx, cudaStream_t st);
 

@@ -55,6 +55,15 @@ struct OpClass {
   long long op_stride(int b) const { return (long long)blocks[b].rp * blocks[b].cp; }
 };
 
+// Pinned host buffers of the environment cache's host tier (api.cu); buffers are re-used between spills.
+struct HostPool {
+  std::vector<std::pair<double*, uint64_t>> free_list;
+  uint64_t total = 0, cap = 0;      // bytes pinned so far / allowed
+  double* get(uint64_t bytes, uint64_t* got);
+  void put(double* p, uint64_t bytes) { if (p) free_list.emplace_back(p, bytes); }
+  ~HostPool();
+};
+
 struct BlockSide {
   bool is_left = true;
   int lo = 0, hi = 0;          // orbitals [lo, hi)
@@ -66,6 +75,13 @@ struct BlockSide {
   std::vector<KindRef> kinds;
   int norb() const { return hi - lo; }
   uint64_t bytes() const { uint64_t b = 0; for (auto& c : cls) if (c) b += (uint64_t)c->elems * 8; return b; }
+  // host tier: a spilled block keeps its layout; the data of all classes sit back to back in one pinned buffer
+  bool spilled = false;
+  double* host = nullptr;
+  uint64_t host_bytes = 0;
+  std::vector<size_t> host_n;         // elements per class in the host buffer
+  std::shared_ptr<HostPool> pool;
+  ~BlockSide() { if (host && pool) pool->put(host, host_bytes); }
 };
 
 struct SiteBlk {
@@ -114,10 +130,12 @@ struct dmrg_ctx {
   // Entries are dropped when a site tensor or bond they depend on changes; total size is capped.
   std::map<int, std::shared_ptr<dmrg::BlockSide>> left_cache, right_cache;
   std::map<int, std::shared_ptr<void>> term_cache;   // bond k -> term groups of the two-site problem (engine.cu)
-  uint64_t cache_bytes() const {
+  std::shared_ptr<dmrg::HostPool> host_pool;         // host tier (cfg.env_host_bytes > 0)
+  int64_t n_spills = 0, n_fetches = 0;
+  uint64_t cache_bytes() const {      // device-resident bytes of the cached blocks
     uint64_t b = 0;
-    for (auto& kv : left_cache) b += kv.second->bytes();
-    for (auto& kv : right_cache) b += kv.second->bytes();
+    for (auto& kv : left_cache) if (!kv.second->spilled) b += kv.second->bytes();
+    for (auto& kv : right_cache) if (!kv.second->spilled) b += kv.second->bytes();
     return b;
   }
   void invalidate_site(int i) {     // site tensor i changed

@@ -131,3 +131,33 @@ def test_su2_sweep_reaches_the_fci_singlet():
     assert min(es[1:]) >= e_singlet - 1e-8
     assert es[-1] - e_singlet <= 1e-2
     sw3.d.close()
+
+
+@pytest.mark.parametrize("su2", [False, True])
+def test_host_tier_of_the_environment_cache(su2):
+    """With a device cap of one byte every cached block that is not in use goes to pinned host memory and comes
+    back when the sweep returns to it: the energies equal those of the all-on-device run bit for bit, and no block
+    is re-blocked (same number of kernel launches)."""
+    import torch
+    from paper_2501_18263_b200.binding import DMRG
+    from paper_2501_18263_b200.sweep import TwoSiteSweep
+    L, N, D, seed = 8, 8, 20, 7
+    T, V = inputs.make_integrals(L, seed)
+    runs = []
+    for kw in (dict(), dict(env_cache_bytes=1, env_host_bytes=1 << 30)):
+        if su2:
+            mps = inputs.make_mps_su2(L, N, D, 1, seed=seed)
+            d = DMRG(L, N // 2, N // 2, su2=True, **kw)
+        else:
+            mps = inputs.make_mps(L, N // 2, N // 2, D, 1, seed=seed)
+            d = DMRG(L, N // 2, N // 2, **kw)
+        sw = TwoSiteSweep(d, T, V, mps, D)
+        es = sw.sweep(nsweeps=2, tol=1e-9, max_iter=200, max_basis=16)
+        runs.append((es, d.stats()))
+        d.close()
+    (e0, s0), (e1, s1) = runs
+    assert e0 == e1
+    assert s0["env_spills"] == 0 and s0["env_fetches"] == 0
+    assert s1["env_spills"] >= L - 3 and s1["env_fetches"] >= L - 3
+    assert s1["env_host_bytes"] <= 1 << 30
+    assert s1["total_launches"] == s0["total_launches"]
