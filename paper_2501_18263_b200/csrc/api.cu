@@ -27,32 +27,20 @@ using namespace dmrg;
   }
 
 namespace dmrg {
-double* HostPool::get(uint64_t bytes, uint64_t* got) {
-  // size classes, so that buffers get re-used: powers of two from 64 KiB, multiples of 256 MiB above that
-  if (bytes > (1ull << 28)) bytes = (bytes + ((1ull << 28) - 1)) & ~((1ull << 28) - 1);
-  else { uint64_t c = 1ull << 16; while (c < bytes) c <<= 1; bytes = c; }
-  int best = -1;
-  for (int i = 0; i < (int)free_list.size(); ++i)
-    if (free_list[i].second >= bytes && (best < 0 || free_list[i].second < free_list[best].second)) best = i;
-  if (best >= 0) {
-    auto pr = free_list[best];
-    free_list.erase(free_list.begin() + best);
-    *got = pr.second;
-    return pr.first;
+bool HostPool::get(size_t npages, std::vector<double*>* out) {
+  out->clear();
+  while (free_pages.size() < npages) {
+    if (total + page_bytes > cap) return false;
+    void* p = nullptr;
+    if (cudaMallocHost(&p, page_bytes) != cudaSuccess) { cudaGetLastError(); return false; }
+    total += page_bytes;
+    free_pages.push_back(static_cast<double*>(p));
   }
-  while (total + bytes > cap && !free_list.empty()) {             // make room from buffers that are too small
-    cudaFreeHost(free_list.back().first);
-    total -= free_list.back().second;
-    free_list.pop_back();
-  }
-  if (total + bytes > cap) return nullptr;
-  void* p = nullptr;
-  if (cudaMallocHost(&p, bytes) != cudaSuccess) { cudaGetLastError(); return nullptr; }
-  total += bytes;
-  *got = bytes;
-  return static_cast<double*>(p);
+  out->assign(free_pages.end() - npages, free_pages.end());
+  free_pages.resize(free_pages.size() - npages);
+  return true;
 }
-HostPool::~HostPool() { for (auto& f : free_list) cudaFreeHost(f.first); }
+HostPool::~HostPool() { for (double* p : free_pages) cudaFreeHost(p); }
 }  // namespace dmrg
 
 extern "C" {
@@ -80,6 +68,9 @@ int dmrg_create(const dmrg_config* cfg, dmrg_ctx** out) {
   if (cfg->env_host_bytes) {
     c->host_pool = std::make_shared<dmrg::HostPool>();
     c->host_pool->cap = cfg->env_host_bytes;
+    // 256 MiB pages for real problems; small caps (tests) get 64 pages
+    uint64_t pb = std::min<uint64_t>(1ull << 28, std::max<uint64_t>(1ull << 16, cfg->env_host_bytes / 64));
+    c->host_pool->page_bytes = pb & ~7ull;
   }
   try {
     if (!std::getenv("DMRG_B200_SERIAL")) c->exec.init();   // debugging aid: every launch in order on one stream
@@ -285,43 +276,57 @@ static uint64_t env_cache_cap(const dmrg_ctx* ctx) {
 }
 
 // ---- host tier of the environment cache (cfg.env_host_bytes) ----
+// copies `n` doubles between a device array and the page list, starting at element `pos` of the paged stream
+static void paged_copy(std::vector<double*>& pages, uint64_t page_elems, uint64_t pos, double* dev, size_t n, bool to_host,
+                       cudaStream_t st) {
+  size_t done = 0;
+  while (done < n) {
+    const uint64_t pg = (pos + done) / page_elems, off = (pos + done) % page_elems;
+    const size_t m = (size_t)std::min<uint64_t>(n - done, page_elems - off);
+    if (to_host) DMRG_CUDA(cudaMemcpyAsync(pages[pg] + off, dev + done, m * 8, cudaMemcpyDeviceToHost, st));
+    else DMRG_CUDA(cudaMemcpyAsync(dev + done, pages[pg] + off, m * 8, cudaMemcpyHostToDevice, st));
+    done += m;
+  }
+}
+
 static bool spill_block(dmrg_ctx* ctx, BlockSide& b, cudaStream_t st) {
   if (b.spilled) return true;
   if (!ctx->host_pool) return false;
-  uint64_t bytes = 0;
-  for (auto& c : b.cls) if (c && c->data.p) bytes += (uint64_t)c->data.n * 8;
-  uint64_t got = 0;
-  double* h = ctx->host_pool->get(std::max<uint64_t>(bytes, 8), &got);
-  if (!h) return false;
+  HostPool& hp = *ctx->host_pool;
+  uint64_t elems = 0;
+  for (auto& c : b.cls) if (c && c->data.p) elems += c->data.n;
+  const uint64_t pe = hp.page_bytes / 8;
+  if (!hp.get((size_t)((elems + pe - 1) / pe), &b.host_pages)) return false;
   b.host_n.assign(b.cls.size(), 0);
-  uint64_t off = 0;
+  uint64_t pos = 0;
   for (size_t i = 0; i < b.cls.size(); ++i) {
     OpClass* c = b.cls[i].get();
     if (!c || !c->data.p) continue;
-    DMRG_CUDA(cudaMemcpyAsync(h + off, c->data.p, c->data.n * 8, cudaMemcpyDeviceToHost, st));
+    paged_copy(b.host_pages, pe, pos, c->data.p, c->data.n, true, st);
     b.host_n[i] = c->data.n;
-    off += c->data.n;
+    pos += c->data.n;
   }
   DMRG_CUDA(cudaStreamSynchronize(st));
   for (auto& c : b.cls) if (c) c->data.release();
-  b.host = h; b.host_bytes = got; b.pool = ctx->host_pool; b.spilled = true;
+  b.pool = ctx->host_pool; b.spilled = true;
   ++ctx->n_spills;
   return true;
 }
 
 static void fetch_block(dmrg_ctx* ctx, BlockSide& b, cudaStream_t st) {
   if (!b.spilled) return;
-  uint64_t off = 0;
+  const uint64_t pe = b.pool->page_bytes / 8;
+  uint64_t pos = 0;
   for (size_t i = 0; i < b.cls.size(); ++i) {
     OpClass* c = b.cls[i].get();
     if (!c || !b.host_n[i]) continue;
     c->data.allocate(&ctx->al, b.host_n[i]);
-    DMRG_CUDA(cudaMemcpyAsync(c->data.p, b.host + off, b.host_n[i] * 8, cudaMemcpyHostToDevice, st));
-    off += b.host_n[i];
+    paged_copy(b.host_pages, pe, pos, c->data.p, b.host_n[i], false, st);
+    pos += b.host_n[i];
   }
   DMRG_CUDA(cudaStreamSynchronize(st));
-  b.pool->put(b.host, b.host_bytes);
-  b.host = nullptr; b.host_bytes = 0; b.pool.reset(); b.spilled = false;
+  b.pool->put(b.host_pages);
+  b.pool.reset(); b.spilled = false;
   ++ctx->n_fetches;
 }
 

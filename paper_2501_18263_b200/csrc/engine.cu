@@ -597,8 +597,6 @@ static void finish_superblock(dmrg_ctx* ctx, std::vector<std::vector<DiagTask>>&
     for (size_t b = 0; b < ctx->psi.size(); ++b) {
       begin[b] = (int)flat.size();
       flat.insert(flat.end(), dtasks[b].begin(), dtasks[b].end());
-      DMRG_REQUIRE(ctx->psi[b].dL <= DIAG_MAX_DIM && ctx->psi[b].dR <= DIAG_MAX_DIM, DMRG_ERR_UNSUPPORTED,
-                   "sector dimension above DIAG_MAX_DIM");
     }
     begin[ctx->psi.size()] = (int)flat.size();
     DevArray<DiagTask> d_tasks;

@@ -116,33 +116,37 @@ __global__ void k_diag(const PsiBlockDev* __restrict__ blocks, const DiagTask* _
   __shared__ double dr[DIAG_T][DIAG_MAXD];
   const PsiBlockDev b = blocks[blockIdx.x];
   const int t0 = task_begin[blockIdx.x], t1 = task_begin[blockIdx.x + 1];
-  const int n = b.rows * b.cols;
-  // each thread owns elements e = tid, tid+blockDim, ... ; accumulate in registers via out (+=)
-  for (long long e = threadIdx.x; e < n; e += blockDim.x)
-    out[b.off_p + (e / b.cols) * b.cols_p + (e % b.cols)] = 0.0;
-  __syncthreads();
-  for (int t = t0; t < t1; ++t) {
-    const DiagTask tk = tasks[t];
-    for (int c0 = 0; c0 < tk.count; c0 += DIAG_T) {
-      const int nc = min(DIAG_T, tk.count - c0);
-      for (int idx = threadIdx.x; idx < nc * b.rows; idx += blockDim.x) {
-        int c = idx / b.rows, a = idx % b.rows;
-        dl[c][a] = tk.L ? tk.L[(long long)(c0 + c) * tk.rsL + (long long)a * tk.ldl + a] : 1.0;
-      }
-      for (int idx = threadIdx.x; idx < nc * b.cols; idx += blockDim.x) {
-        int c = idx / b.cols, a = idx % b.cols;
-        dr[c][a] = tk.R ? tk.R[(long long)(c0 + c) * tk.rsR + (long long)a * tk.ldr + a] : 1.0;
-      }
+  // sectors larger than DIAG_MAXD are covered by (row range) x (column range) panels
+  for (int r0 = 0; r0 < b.rows; r0 += DIAG_MAXD)
+    for (int q0 = 0; q0 < b.cols; q0 += DIAG_MAXD) {
+      const int nr = min(DIAG_MAXD, b.rows - r0), nq = min(DIAG_MAXD, b.cols - q0);
+      const int n = nr * nq;
+      for (int e = threadIdx.x; e < n; e += blockDim.x)
+        out[b.off_p + (long long)(r0 + e / nq) * b.cols_p + (q0 + e % nq)] = 0.0;
       __syncthreads();
-      for (int e = threadIdx.x; e < n; e += blockDim.x) {
-        int r = e / b.cols, c = e % b.cols;
-        double s = 0.0;
-        for (int q = 0; q < nc; ++q) s = fma(dl[q][r], dr[q][c], s);
-        out[b.off_p + (long long)r * b.cols_p + c] += tk.alpha * s;
+      for (int t = t0; t < t1; ++t) {
+        const DiagTask tk = tasks[t];
+        for (int c0 = 0; c0 < tk.count; c0 += DIAG_T) {
+          const int nc = min(DIAG_T, tk.count - c0);
+          for (int idx = threadIdx.x; idx < nc * nr; idx += blockDim.x) {
+            int c = idx / nr, a = r0 + idx % nr;
+            dl[c][idx % nr] = tk.L ? tk.L[(long long)(c0 + c) * tk.rsL + (long long)a * tk.ldl + a] : 1.0;
+          }
+          for (int idx = threadIdx.x; idx < nc * nq; idx += blockDim.x) {
+            int c = idx / nq, a = q0 + idx % nq;
+            dr[c][idx % nq] = tk.R ? tk.R[(long long)(c0 + c) * tk.rsR + (long long)a * tk.ldr + a] : 1.0;
+          }
+          __syncthreads();
+          for (int e = threadIdx.x; e < n; e += blockDim.x) {
+            int r = e / nq, c = e % nq;
+            double s = 0.0;
+            for (int q = 0; q < nc; ++q) s = fma(dl[q][r], dr[q][c], s);
+            out[b.off_p + (long long)(r0 + r) * b.cols_p + (q0 + c)] += tk.alpha * s;
+          }
+          __syncthreads();
+        }
       }
-      __syncthreads();
     }
-  }
 }
 
 __global__ void k_reduce_partials(const RedDesc* __restrict__ ds) {

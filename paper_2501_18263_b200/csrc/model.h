@@ -55,12 +55,14 @@ struct OpClass {
   long long op_stride(int b) const { return (long long)blocks[b].rp * blocks[b].cp; }
 };
 
-// Pinned host buffers of the environment cache's host tier (api.cu); buffers are re-used between spills.
+// Pinned host memory of the environment cache's host tier (api.cu): fixed-size pages, pinned on first use and kept
+// until the context dies (pinning costs ~0.3 s per GB, a copy into a pinned page runs at PCIe speed), so any free
+// page fits any block.
 struct HostPool {
-  std::vector<std::pair<double*, uint64_t>> free_list;
-  uint64_t total = 0, cap = 0;      // bytes pinned so far / allowed
-  double* get(uint64_t bytes, uint64_t* got);
-  void put(double* p, uint64_t bytes) { if (p) free_list.emplace_back(p, bytes); }
+  std::vector<double*> free_pages;
+  uint64_t page_bytes = 0, total = 0, cap = 0;      // bytes pinned so far / allowed
+  bool get(size_t npages, std::vector<double*>* out);
+  void put(std::vector<double*>& pages) { for (double* p : pages) free_pages.push_back(p); pages.clear(); }
   ~HostPool();
 };
 
@@ -75,13 +77,12 @@ struct BlockSide {
   std::vector<KindRef> kinds;
   int norb() const { return hi - lo; }
   uint64_t bytes() const { uint64_t b = 0; for (auto& c : cls) if (c) b += (uint64_t)c->elems * 8; return b; }
-  // host tier: a spilled block keeps its layout; the data of all classes sit back to back in one pinned buffer
+  // host tier: a spilled block keeps its layout; the data of all classes sit back to back in pinned pages
   bool spilled = false;
-  double* host = nullptr;
-  uint64_t host_bytes = 0;
-  std::vector<size_t> host_n;         // elements per class in the host buffer
+  std::vector<double*> host_pages;
+  std::vector<size_t> host_n;         // elements per class in the host copy
   std::shared_ptr<HostPool> pool;
-  ~BlockSide() { if (host && pool) pool->put(host, host_bytes); }
+  ~BlockSide() { if (pool) pool->put(host_pages); }
 };
 
 struct SiteBlk {

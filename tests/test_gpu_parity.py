@@ -255,3 +255,27 @@ def test_input_errors_are_reported():
     with pytest.raises(DMRGError):
         d.env_build(7)
     d.close()
+
+
+def test_diag_of_sectors_wider_than_one_panel():
+    """k_diag covers sectors above its 640-wide shared-memory panel in several panels (dims 705 here): the diagonal
+    must equal <e_i|H_eff|e_i> from the (oracle-checked) apply at sampled positions in every panel of the
+    largest blocks, and at random positions."""
+    import torch
+    L, n_el, D = 16, 8, 6000
+    T, V = inputs.make_integrals(L, 77)
+    mps = inputs.make_mps(L, n_el, n_el, D, L // 2, seed=77)
+    d = _gpu(T, V, mps)
+    blocks, n = d.psi_layout()
+    big = max(blocks, key=lambda b: min(b.dL, b.dR))
+    assert big.dL > 640 and big.dR > 640
+    dg = d.heff_diag().cpu().numpy()
+    rng = np.random.default_rng(0)
+    picks = [big.off + r * big.dR + c for r in (0, 639, 640, big.dL - 1) for c in (0, 639, 640, big.dR - 1)]
+    picks += [int(i) for i in rng.integers(0, n, size=8)]
+    for i in picks:
+        e = torch.zeros(n, dtype=torch.float64, device="cuda")
+        e[i] = 1.0
+        hi = float(d.heff_apply(e)[i])
+        assert abs(hi - dg[i]) <= 1e-11 * max(1.0, abs(hi)), (i, hi, dg[i])
+    d.close()
