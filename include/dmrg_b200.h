@@ -60,7 +60,9 @@ typedef struct {
                            only (n_up == n_dn): bond sectors are then labelled (N, 2S) in the q_up/q_dn arrays */
   int32_t device;       /* CUDA device ordinal */
   uint64_t workspace_bytes; /* cap for the intermediate (O_L.psi) buffer; 0 = library default */
-  uint64_t env_cache_bytes; /* cap for cached environment blocks (sweeps re-use them); 0 = 1/8 of device memory */
+  uint64_t env_cache_bytes; /* device cap for cached environment blocks (sweeps re-use them); 0 = 1/8 of device memory.
+                               Over the cap the cached block farthest from the current bond is moved to the host tier
+                               (env_host_bytes) or dropped; the two blocks in use do not count as removable */
   dmrg_alloc_fn alloc;
   dmrg_free_fn free;
   void* alloc_user;

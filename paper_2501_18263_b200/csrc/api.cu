@@ -341,8 +341,8 @@ static void cache_enforce(dmrg_ctx* ctx, int near, cudaStream_t st) {
     for (int side = 0; side < 2; ++side)
       for (auto& kv : (side == 0 ? ctx->left_cache : ctx->right_cache)) {
         if (kv.second->spilled) continue;
+        if (kv.second == ctx->left || kv.second == ctx->right) continue;    // in use: neither counted nor moved
         res += kv.second->bytes();
-        if (kv.second == ctx->left || kv.second == ctx->right) continue;
         const int dist = std::abs(kv.first - near);
         if (dist > far_dist) { far_dist = dist; far = kv.second; far_left = side == 0; far_key = kv.first; }
       }
@@ -353,9 +353,8 @@ static void cache_enforce(dmrg_ctx* ctx, int near, cudaStream_t st) {
 }
 
 static void cache_put(dmrg_ctx* ctx, bool left, int key, const std::shared_ptr<BlockSide>& b, cudaStream_t st) {
-  if (!ctx->host_pool && ctx->cache_bytes() + b->bytes() > env_cache_cap(ctx)) return;   // no host tier: first come
   (left ? ctx->left_cache : ctx->right_cache)[key] = b;
-  if (ctx->host_pool) cache_enforce(ctx, key, st);
+  cache_enforce(ctx, key, st);
 }
 
 static void build_side(dmrg_ctx* ctx, bool left, int upto, cudaStream_t st, double* flops_last) {
