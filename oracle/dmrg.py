@@ -457,6 +457,11 @@ def davidson(apply, diag, v0, tol=1e-10, max_iter=200, max_basis=20):
     orthogonalise t against V twice (classical Gram-Schmidt), normalise, append; restart to
     [x] when the basis reaches max_basis.  Returns (theta, x, iterations, |r|) with
     iterations = number of operator applications.
+
+    Pinned: the converged energy equals the brute-force FCI ground-state energy at untruncated
+    bond dimension (tests/test_oracle_dmrg.py).  Parity unpinned: the iterate-by-iterate
+    trajectory (energy / residual after a fixed number of iterations) has no value outside this
+    file to compare with; the paper names no eigensolver (R13).
     """
     v = np.asarray(v0, dtype=np.float64)
     v = v / np.linalg.norm(v)
