@@ -260,7 +260,13 @@ k_grouped_gemm(const GOut* __restrict__ outs, const GSeg* __restrict__ segs, con
   int stage = 0;
   unsigned phase = 0;
 
+  // Register split (12-warp instance only: warpgroups 0-1 = consumers, warpgroup 2 = producers): the
+  // producers hand most of their registers to the consumers, whose 128 accumulator registers otherwise leave
+  // no room to keep the fragment addresses and a full set of fragments live (at the 168-register cap ptxas
+  // re-derives the shared-memory addresses at every k-step and funnels the A fragments through one register).
+  constexpr bool REGSPLIT = (NCW == 8 && NP == 4 && MINB == 1);
   if (warp >= NCW) {
+    if constexpr (REGSPLIT) asm volatile("setmaxnreg.dec.sync.aligned.u32 72;\n" ::);
     // ------------------------------------------------ producers ------------------------------------------------
     // (every tile of the list has at least one k-chunk: the planner emits no tiles for empty outputs)
     const int pt = tid - 32 * NCW;
@@ -308,6 +314,7 @@ k_grouped_gemm(const GOut* __restrict__ outs, const GSeg* __restrict__ segs, con
 
   // ---------------------------------------------------- consumers ----------------------------------------------------
   // One stream of stages; tile boundaries are flags in the stage meta.
+  if constexpr (REGSPLIT) asm volatile("setmaxnreg.inc.sync.aligned.u32 216;\n" ::);
   const int wm0 = (warp / WC) * WM, wn0 = (warp % WC) * WN;
   const int lr = lane >> 2, lk = lane & 3;
   double acc[FA][FB][2];
