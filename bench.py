@@ -302,9 +302,9 @@ def run_ours(args):
     # DRAM bytes per launch of the dominant kernel from the committed ncu --set full capture of this workload
     # (profiles/r01_gemm128_full.md: dram__bytes_read.sum + dram__bytes_write.sum); only known for the default config.
     if cfg == 3 and not su2 and not args.D:
-        traffic_detail = {"phase1_bytes_per_launch": [25.19e9, 43.59e9], "phase2_bytes_per_launch": [28.05e9],
+        traffic_detail = {"phase1_bytes_per_launch": [26.02e9, 45.69e9], "phase2_bytes_per_launch": [28.67e9],
                           "source": "profiles/r01_gemm128_full.md (three captured launches)"}
-        traffic = (25.19e9 + 43.59e9 + 28.05e9) / 3
+        traffic = (26.02e9 + 45.69e9 + 28.67e9) / 3
     else:
         traffic_detail, traffic = None, None
     if rank == 0:
