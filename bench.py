@@ -243,8 +243,17 @@ def run_ours(args):
             a = dom.setdefault(r["phase"], [0, 0.0, 0.0])
             a[0] += 1; a[1] += r["flops"]; a[2] += r["ms"]
     tot_ms = sum(r["ms"] for r in rec) or 1.0
+    # every tile shape, serialised: {"<phase>:<rows>x<cols>": [ms, TFLOP/s]} (shape = 3 * row class + col class)
+    per_shape = {}
+    for r in rec:
+        if 0 <= r["shape"] < 9 and r["flops"] > 0:
+            key = "%d:%dx%d" % (r["phase"], (32, 64, 128)[r["shape"] // 3], (32, 64, 128)[r["shape"] % 3])
+            a = per_shape.setdefault(key, [0.0, 0.0])
+            a[0] += r["ms"]; a[1] += r["flops"]
+    per_shape = {k: [round(v[0], 3), round(v[1] / v[0] * 1e-9, 2)] for k, v in sorted(per_shape.items()) if v[0] > 0}
     dominant = {"kernel": "k_grouped_gemm<128,128> (tile shape 128x128)",
                 "share_of_serial_step": sum(v[2] for v in dom.values()) / tot_ms,
+                "serial_ms_and_tflops_per_shape": per_shape,
                 "per_phase": {str(k): {"launches": v[0], "avg_ms": v[2] / v[0], "flops_per_launch": v[1] / v[0],
                                        "tflops": v[1] / v[2] * 1e-9} for k, v in dom.items() if v[0]}}
     dom_fl = sum(v[1] for v in dom.values())

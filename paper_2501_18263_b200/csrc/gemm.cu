@@ -260,13 +260,18 @@ k_grouped_gemm(const GOut* __restrict__ outs, const GSeg* __restrict__ segs, con
   int stage = 0;
   unsigned phase = 0;
 
-  // Register split (12-warp instance only: warpgroups 0-1 = consumers, warpgroup 2 = producers): the
-  // producers hand most of their registers to the consumers, whose 128 accumulator registers otherwise leave
-  // no room to keep the fragment addresses and a full set of fragments live (at the 168-register cap ptxas
+  // Register split (instances with 64x32 warp tiles whose consumer and producer warps are whole warpgroups):
+  // the producers hand most of their registers to the consumers, whose 128 accumulator registers otherwise
+  // leave no room to keep the fragment addresses and a full set of fragments live (at the launch-time cap ptxas
   // re-derives the shared-memory addresses at every k-step and funnels the A fragments through one register).
-  constexpr bool REGSPLIT = (NCW == 8 && NP == 4 && MINB == 1);
+  // The CTA's total stays what it was launched with: NP * (BASE - PREG) = NCW * (CREG - BASE).
+  constexpr bool REGSPLIT = (WM == 64 && WN == 32 && NCW % 4 == 0 && NP % 4 == 0);
+  constexpr int BASEREG = (65536 / (32 * (NCW + NP) * MINB)) / 8 * 8;   // what __launch_bounds__ lets ptxas use
+  constexpr int PREG = BASEREG >= 160 ? 72 : 56;
+  constexpr int CREG = (BASEREG + (BASEREG - PREG) * NP / NCW) / 8 * 8;
+  static_assert(!REGSPLIT || (CREG <= 232 && NP * PREG + NCW * CREG <= (NCW + NP) * BASEREG), "register split");
   if (warp >= NCW) {
-    if constexpr (REGSPLIT) asm volatile("setmaxnreg.dec.sync.aligned.u32 72;\n" ::);
+    if constexpr (REGSPLIT) asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;\n" ::"n"(PREG));
     // ------------------------------------------------ producers ------------------------------------------------
     // (every tile of the list has at least one k-chunk: the planner emits no tiles for empty outputs)
     const int pt = tid - 32 * NCW;
@@ -314,7 +319,7 @@ k_grouped_gemm(const GOut* __restrict__ outs, const GSeg* __restrict__ segs, con
 
   // ---------------------------------------------------- consumers ----------------------------------------------------
   // One stream of stages; tile boundaries are flags in the stage meta.
-  if constexpr (REGSPLIT) asm volatile("setmaxnreg.inc.sync.aligned.u32 216;\n" ::);
+  if constexpr (REGSPLIT) asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;\n" ::"n"(CREG));
   const int wm0 = (warp / WC) * WM, wn0 = (warp % WC) * WN;
   const int lr = lane >> 2, lk = lane & 3;
   double acc[FA][FB][2];
@@ -404,10 +409,10 @@ using S32x64   = Cfg<32, 64, 1, 2, 2, 6, 3>;   // 32x32
 using S32x128  = Cfg<32, 128, 1, 4, 2, 4, 2>;  // 32x32
 using S64x32   = Cfg<64, 32, 2, 1, 2, 6, 3>;   // 32x32
 using S64x64   = Cfg<64, 64, 2, 2, 4, 4, 2>;   // 32x32
-using S64x128  = Cfg<64, 128, 1, 4, 2, 3, 2>;  // 64x32
+using S64x128  = Cfg<64, 128, 1, 4, 4, 3, 2>;  // 64x32, register split 56 / 200
 using S128x32  = Cfg<128, 32, 4, 1, 2, 4, 2>;  // 32x32
-using S128x64  = Cfg<128, 64, 2, 2, 2, 3, 2>;  // 64x32
-using S128x128 = Cfg<128, 128, 2, 4, 4, 5, 1>; // 64x32
+using S128x64  = Cfg<128, 64, 2, 2, 4, 3, 2>;  // 64x32, register split 56 / 200
+using S128x128 = Cfg<128, 128, 2, 4, 4, 5, 1>; // 64x32, register split 72 / 216
 
 }  // namespace
 
