@@ -203,6 +203,19 @@ int dmrg_stats(dmrg_ctx* ctx, dmrg_stats_t* out);
 int dmrg_env_export(dmrg_ctx* ctx, int32_t side, int32_t kind, int32_t i, int32_t j,
                     double* h_out, int64_t* D);
 
+/* One sector block of EVERY operator of a carried class (parity tests at sizes where the dense matrices of
+ * dmrg_env_export are too large: BASELINE configs 3 and 4).  U(1)xU(1) contexts: `kind` as in dmrg_env_export and
+ * `d2S` is ignored.  SU(2) contexts: kind 0 H, 1 C (rank 1/2), 2 A^0, 3 A^1, 4 B^0, 5 B^1, 6 S~ (rank 1/2) — the reduced
+ * elements X_red[S',S] of <S'M'|X^k_q|SM> = <S M; k q|S' M'> X_red[S',S] — and d2S = 2S' - 2S selects the
+ * class.  The block is chosen by the label of its INPUT sector, (q_up, q_dn) resp. (N, 2S), in the convention of
+ * dmrg_psi_block: left block = content of the block, right block = label of the bond (electrons LEFT of it).
+ * Returns *nops, *rows (output sector), *cols (input sector) and, if h_out != NULL, the nops x rows x cols
+ * row-major array; *rows = *cols = 0 if the class has no block with that input sector.  Operator order inside a
+ * class: C, S: orbitals ascending (S: the orbitals OUTSIDE the block); A_upup, A_dndn, A^1: pairs i < j, i-major;
+ * A^0: pairs i <= j, i-major; A_updn, B_*, B^0, B^1: (i, j) row-major over the block's orbitals. */
+int dmrg_env_export_block(dmrg_ctx* ctx, int32_t side, int32_t kind, int32_t d2S, int32_t qin_a, int32_t qin_b,
+                          int32_t* nops, int32_t* rows, int32_t* cols, double* h_out);
+
 /* The factor F of PAPER.md Eq. (10)-(11) (host; doubled-spin arguments): *h_F_ninej = the rescaled Wigner 9j
  * closed form sqrt((2Sa'+1)(2Sk'+1)(2Sg+1)(2k+1)) {Sa Sk Sg; kL kk k; Sa' Sk' Sg'}, *h_F_contraction = the contraction
  * of six Clebsch-Gordan tensors of PAPER.md Fig. 4 from the library's own CG table (the table all SU(2) task

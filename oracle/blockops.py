@@ -78,13 +78,20 @@ def identity(sectors) -> BlockOp:
     return BlockOp({(q, q): np.eye(d) for q, d in sectors.items()})
 
 
-def product(X1: BlockOp, X2: BlockOp, coef: float = 1.0) -> ProdOp:
-    """Matrix of coef * X1 X2 (X1 on B1 written first, X2 on B2) on the product basis."""
+def product(X1: BlockOp, X2: BlockOp, coef: float = 1.0, keep=None) -> ProdOp:
+    """Matrix of coef * X1 X2 (X1 on B1 written first, X2 on B2) on the product basis.
+
+    keep: optional set of product sector keys (q1, q2).  Only the sub-blocks whose out key or in
+    key is in the set are formed (the others are simply absent, as for a restricted operator);
+    None = all of them.  Used by oracle/lean.py to evaluate H_eff psi on chosen output blocks.
+    """
     p2 = X2.parity()
     out = ProdOp()
     for (q1o, q1i), m1 in X1.items():
         sg = -1.0 if (p2 and (qnum(q1i) & 1)) else 1.0
         for (q2o, q2i), m2 in X2.items():
+            if keep is not None and (q1o, q2o) not in keep and (q1i, q2i) not in keep:
+                continue
             out[((q1o, q2o), (q1i, q2i))] = (coef * sg) * np.kron(m1, m2)
     return out
 

@@ -39,7 +39,10 @@ from __future__ import annotations
 
 import numpy as np
 
-from .blockops import BlockOp, ProdOp, identity, lincomb, product, project, qadd, qnum, qsub
+import functools
+
+from .blockops import BlockOp, ProdOp, identity, lincomb, project, qadd, qnum, qsub
+from .blockops import product as _product
 
 SITE_Q = ((0, 0), (0, 1), (1, 0), (1, 1))  # s = 0, dn, up, up+dn  ->  (n_up, n_dn)
 
@@ -158,23 +161,29 @@ def comp_Q_many(B: Block, w, pairs):
 # ---------------------------------------------------------------------------------------------
 
 class Enlarged:
-    def __init__(self, B1: Block, B2: Block):
+    def __init__(self, B1: Block, B2: Block, keep=None):
         self.B1, self.B2 = B1, B2
         self.orbs = B1.orbs + B2.orbs
         self.ops = {}
         self.I1 = identity(B1.sectors)
         self.I2 = identity(B2.sectors)
+        self.keep = keep
 
     def spin_orbs(self):
         return [2 * i + s for i in self.orbs for s in (0, 1)]
 
     def identity(self) -> ProdOp:
-        return product(self.I1, self.I2)
+        return _product(self.I1, self.I2, keep=self.keep)
 
 
-def enlarge(B1: Block, B2: Block, T, w, ext_orbs, want_normal=True, want_H=True) -> Enlarged:
-    """Operators of B = B1 u B2 (B1 left of B2) as ProdOps; S_p for p over ext_orbs."""
-    E = Enlarged(B1, B2)
+def enlarge(B1: Block, B2: Block, T, w, ext_orbs, want_normal=True, want_H=True, keep=None) -> Enlarged:
+    """Operators of B = B1 u B2 (B1 left of B2) as ProdOps; S_p for p over ext_orbs.
+
+    keep: optional set of product sector keys; every Kronecker product below then forms only the
+    sub-blocks that touch one of them (blockops.product).  The formulas are unchanged.
+    """
+    product = functools.partial(_product, keep=keep)
+    E = Enlarged(B1, B2, keep)
     I1, I2 = E.I1, E.I2
     so1, so2 = B1.spin_orbs(), B2.spin_orbs()
     in1, in2 = set(so1), set(so2)
@@ -341,17 +350,22 @@ class TwoSiteOracle:
         self._terms = None
 
     # ---- superblock terms: bipartition identity between L' = L u k and R' = k+1 u R ----
-    def terms(self):
-        """List of (X_L', X_R', hc) with H_eff = sum X_L' (x) X_R' (+ transpose if hc)."""
-        if self._terms is not None:
+    def terms(self, keepL=None, keepR=None):
+        """List of (X_L', X_R', hc) with H_eff = sum X_L' (x) X_R' (+ transpose if hc).
+
+        keepL / keepR: optional sets of L' / R' product sector keys; the enlarged operators are then
+        formed only on the sub-blocks that touch them (not cached).  None = everything (cached).
+        """
+        lean = keepL is not None or keepR is not None
+        if self._terms is not None and not lean:
             return self._terms
         k, L = self.k, self.L
         s1 = site_block(k - 1, self.T, self.w, L)
         s2 = site_block(k, self.T, self.w, L)
         orbsL = list(range(0, k))        # orbitals of L'
         orbsR = list(range(k, L))        # orbitals of R'
-        EL = enlarge(self.Lblock, s1, self.T, self.w, orbsR)
-        ER = enlarge(s2, self.Rblock, self.T, self.w, orbsL)
+        EL = enlarge(self.Lblock, s1, self.T, self.w, orbsR, keep=keepL)
+        ER = enlarge(s2, self.Rblock, self.T, self.w, orbsL, keep=keepR)
         soL = EL.spin_orbs()
         soR = ER.spin_orbs()
         IL, IR = EL.identity(), ER.identity()
@@ -372,7 +386,8 @@ class TwoSiteOracle:
         for (p, q), Qc in zip(prs, comp_Q_many(ERb, self.w, prs)):
             if Qc:
                 terms.append((EL.ops[("B", p, q)], Qc, False))
-        self._terms = terms
+        if not lean:
+            self._terms = terms
         return terms
 
     # ---- psi layout ----
@@ -399,10 +414,15 @@ class TwoSiteOracle:
     def apply(self, v):
         psi = self.unflatten(np.asarray(v, dtype=np.float64))
         out = {kk: np.zeros_like(m) for kk, m in psi.items()}
+        self._accumulate(self.terms(), psi, out)
+        return self.flatten(out)
+
+    def _accumulate(self, terms, psi, out):
+        """out{key} += sum_terms (X_L' (x) X_R' psi){key} for the keys present in `out`."""
         by_left = {}
         for (kl, kr), m in psi.items():
             by_left.setdefault(kl, []).append((kr, m))
-        for XL, XR, hc in self.terms():
+        for XL, XR, hc in terms:
             pR = XR.parity()
             r_by_in, r_by_out = {}, {}
             for (kro, kri), mR in XR.items():
@@ -422,7 +442,6 @@ class TwoSiteOracle:
                             o = out.get((kli, kri))
                             if o is not None:
                                 o += sg * (mL.T @ x @ mR)
-        return self.flatten(out)
 
     def diag(self):
         """Diagonal of H_eff in the psi layout (Davidson preconditioner, DESIGN.md App. E)."""

@@ -22,7 +22,7 @@ EXPORTS = [
     "dmrg_mps_set_site", "dmrg_env_build", "dmrg_renormalize", "dmrg_psi_layout", "dmrg_heff_apply",
     "dmrg_heff_diag", "dmrg_davidson", "dmrg_heff_apply_host", "dmrg_davidson_host", "dmrg_stats",
     "dmrg_env_export", "dmrg_fp64_peak", "dmrg_apply_profile", "dmrg_mps_set_site_su2", "dmrg_su2_f_factor",
-    "dmrg_mps_update_bond", "dmrg_set_shard", "dmrg_shard_info",
+    "dmrg_mps_update_bond", "dmrg_set_shard", "dmrg_shard_info", "dmrg_env_export_block",
 ]
 
 REDUCE_FN = C.CFUNCTYPE(C.c_int, C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p)
@@ -96,6 +96,7 @@ def load_library(build_if_missing: bool = True):
     lib.dmrg_davidson_host.argtypes = [vp, vp, C.c_double, i32, i32, dp, C.POINTER(i32), dp, vp]
     lib.dmrg_stats.argtypes = [vp, C.POINTER(Stats)]
     lib.dmrg_env_export.argtypes = [vp, i32, i32, i32, i32, vp, C.POINTER(i64)]
+    lib.dmrg_env_export_block.argtypes = [vp, i32, i32, i32, i32, i32, C.POINTER(i32), C.POINTER(i32), C.POINTER(i32), vp]
     lib.dmrg_fp64_peak.argtypes = [vp, dp, vp]
     lib.dmrg_apply_profile.argtypes = [vp, vp, vp, i32, C.POINTER(LaunchInfo), C.POINTER(i32), vp]
     for name in EXPORTS:
@@ -317,6 +318,19 @@ class DMRG:
         self._check(self.lib.dmrg_env_export(self.ctx, side, kind, i, j, None, C.byref(D)))
         out = np.zeros((D.value, D.value))
         self._check(self.lib.dmrg_env_export(self.ctx, side, kind, i, j, _np_ptr(out), C.byref(D)))
+        return out
+
+    def env_export_block(self, side, kind, qin, d2S=0):
+        """(nops, rows, cols) array of one sector block of every operator of a class, or None if the class has no
+        block with input sector `qin` (label convention of dmrg_psi_block)."""
+        n, r, c = C.c_int32(), C.c_int32(), C.c_int32()
+        self._check(self.lib.dmrg_env_export_block(self.ctx, side, kind, d2S, qin[0], qin[1], C.byref(n), C.byref(r),
+                                                   C.byref(c), None))
+        if r.value == 0 or c.value == 0 or n.value == 0:
+            return None
+        out = np.empty((n.value, r.value, c.value))
+        self._check(self.lib.dmrg_env_export_block(self.ctx, side, kind, d2S, qin[0], qin[1], C.byref(n), C.byref(r),
+                                                   C.byref(c), _np_ptr(out)))
         return out
 
     def fp64_peak(self):

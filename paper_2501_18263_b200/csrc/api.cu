@@ -268,6 +268,20 @@ int dmrg_mps_set_site_su2(dmrg_ctx* ctx, int32_t site, int32_t canonical, int32_
   return set_site_impl(ctx, site, canonical, nblocks, qin, m, qout, blk_off, h_data, stream);
 }
 
+// dmrg_env_build / dmrg_renormalize: while the environments and the plan are being replaced there is no prepared
+// problem; if the call fails half way the context stays in that state (k = 0) instead of pointing at stale blocks.
+struct PreparedGuard {
+  dmrg_ctx* ctx;
+  bool ok = false;
+  ~PreparedGuard() {
+    if (ok) return;
+    ctx->k = 0;
+    ctx->apply_plan.clear();
+    ctx->left.reset();
+    ctx->right.reset();
+  }
+};
+
 static uint64_t env_cache_cap(const dmrg_ctx* ctx) {
   if (ctx->cfg.env_cache_bytes) return ctx->cfg.env_cache_bytes;
   size_t fr = 0, tot = 0;
@@ -392,6 +406,7 @@ int dmrg_env_build(dmrg_ctx* ctx, int32_t k, void* stream) {
   DMRG_REQUIRE(ctx->have_integrals && !ctx->bond.empty(), DMRG_ERR_ARG, "env_build: integrals and sectors first");
   DMRG_REQUIRE(k >= 1 && k + 1 <= ctx->L, DMRG_ERR_ARG, "env_build: bond out of range");
   auto t0 = std::chrono::steady_clock::now();
+  PreparedGuard guard{ctx};   // no prepared problem unless this call succeeds
   ctx->apply_plan.clear();
   if (ctx->left) drop_presummed(*ctx->left, ctx->su2());      // they may stay in the cache: carried operators only
   if (ctx->right) drop_presummed(*ctx->right, ctx->su2());
@@ -404,6 +419,7 @@ int dmrg_env_build(dmrg_ctx* ctx, int32_t k, void* stream) {
   ctx->k = k;
   if (ctx->su2()) prepare_superblock_su2(ctx, st); else prepare_superblock(ctx, st);
   ctx->stats.last_build_ms = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t0).count();
+  guard.ok = true;
   API_END
 }
 
@@ -414,6 +430,9 @@ int dmrg_renormalize(dmrg_ctx* ctx, int32_t direction, void* stream) {
   auto t0 = std::chrono::steady_clock::now();
   const int k = ctx->k;
   double fl = 0;
+  DMRG_REQUIRE(direction == 0 || direction == 1, DMRG_ERR_ARG, "renormalize: direction must be 0 or 1");
+  DMRG_REQUIRE(direction == 0 ? k + 2 <= ctx->L : k - 1 >= 1, DMRG_ERR_ARG, "renormalize: already at the end of the chain");
+  PreparedGuard guard{ctx};   // no prepared problem unless this call succeeds
   ctx->apply_plan.clear();
   drop_presummed(*ctx->left, ctx->su2());
   drop_presummed(*ctx->right, ctx->su2());
@@ -444,6 +463,7 @@ int dmrg_renormalize(dmrg_ctx* ctx, int32_t direction, void* stream) {
   ctx->stats.flops_renorm = fl;
   if (ctx->su2()) prepare_superblock_su2(ctx, st); else prepare_superblock(ctx, st);
   ctx->stats.last_build_ms = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t0).count();
+  guard.ok = true;
   API_END
 }
 
@@ -596,7 +616,7 @@ static void davidson_padded(dmrg_ctx* ctx, double* x_p, double tol, int max_iter
     launch_combine(V, n, d_small + 64, m, n, xr, st);
     launch_combine(W, n, d_small + 64, m, n, hx, st);
     double* r = ctx->psi_in_p.p;   // scratch: overwritten by the next apply anyway
-    launch_residual_precond(xr, hx, ctx->diag_p.p, theta - ctx->e_core, r, t, n, st);
+    launch_residual_precond(xr, hx, ctx->diag_p.p, theta, theta - ctx->e_core, r, t, n, st);
     ctx->launches += 3;
     double r2;
     dots(r, r, 1, &r2);
@@ -755,6 +775,43 @@ int dmrg_env_export(dmrg_ctx* ctx, int32_t side, int32_t kind, int32_t i, int32_
         for (int c = 0; c < cb.cols; ++c)
           h_out[(start[cb.so] + r) * D + start[cb.si] + c] = h[(size_t)r * cb.cp + c];
     }
+  }
+  API_END
+}
+
+int dmrg_env_export_block(dmrg_ctx* ctx, int32_t side, int32_t kind, int32_t d2S, int32_t qa, int32_t qb, int32_t* nops,
+                          int32_t* rows, int32_t* cols, double* h_out) {
+  API_BEGIN
+  DMRG_REQUIRE(ctx->k > 0 && (side == 0 || side == 1) && nops && rows && cols, DMRG_ERR_ARG, "env_export_block: bad arguments");
+  const BlockSide& B = side == 0 ? *ctx->left : *ctx->right;
+  const OpClass* C = nullptr;
+  int ca = qa, cb = qb;     // the block's own content
+  if (ctx->su2()) {
+    DMRG_REQUIRE(kind >= 0 && kind <= 6, DMRG_ERR_ARG, "env_export_block: kind out of range");
+    const auto& kr = B.kinds[kind + 1];                 // su2e::SKind without SK_ID
+    DMRG_REQUIRE(d2S >= -kr.k2 && d2S <= kr.k2 && !((d2S + kr.k2) & 1), DMRG_ERR_ARG, "env_export_block: d2S is not a spin change of this kind");
+    C = B.cls[kr.cids[(d2S + kr.k2) / 2]].get();
+    if (side == 1) ca = ctx->cfg.n_up + ctx->cfg.n_dn - qa;
+  } else {
+    static const int kmap[11] = {K_H, K_CU, K_CD, K_AUU, K_AUD, K_ADD, K_BUU, K_BUD, K_BDD, K_SU, K_SD};
+    DMRG_REQUIRE(kind >= 0 && kind <= 10, DMRG_ERR_ARG, "env_export_block: kind out of range");
+    C = B.cls[kmap[kind]].get();
+    if (side == 1) { ca = ctx->cfg.n_up - qa; cb = ctx->cfg.n_dn - qb; }
+  }
+  DMRG_REQUIRE(C && C->data.p, DMRG_ERR_ARG, "env_export_block: class not resident");
+  *nops = C->nops; *rows = 0; *cols = 0;
+  const int si = B.sec.find(ca, cb);
+  const int b = si >= 0 ? C->blk_of_in[si] : -1;
+  if (b < 0) return DMRG_OK;
+  const ClsBlock& cb_ = C->blocks[b];
+  *rows = cb_.rows; *cols = cb_.cols;
+  if (h_out && C->nops > 0) {
+    std::vector<double> h((size_t)C->nops * cb_.rp * cb_.cp);
+    DMRG_CUDA(cudaMemcpy(h.data(), C->ptr(b, 0), h.size() * 8, cudaMemcpyDeviceToHost));
+    for (int o = 0; o < C->nops; ++o)
+      for (int r = 0; r < cb_.rows; ++r)
+        std::memcpy(h_out + ((size_t)o * cb_.rows + r) * cb_.cols, h.data() + ((size_t)o * cb_.rp + r) * cb_.cp,
+                    sizeof(double) * cb_.cols);
   }
   API_END
 }

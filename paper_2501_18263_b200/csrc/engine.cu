@@ -101,7 +101,6 @@ int SiteOpTable::parity(int id) const {
   return 0;
 }
 
-// product of the elementary site operators in `ops` (leftmost first); returns interned id or -1
 // product of the elementary site operators in `ops` (leftmost first); returns interned id or -1.
 // All strings of up to four elementary operators are interned when the table is built, so this is a
 // read-only lookup (the term enumeration calls it from several threads).

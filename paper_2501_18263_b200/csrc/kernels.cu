@@ -97,12 +97,12 @@ __global__ void k_add_const(double a, double* __restrict__ y, long long n) {
 }
 
 __global__ void k_resid(const double* __restrict__ x, const double* __restrict__ hx,
-                        const double* __restrict__ d, double theta, double* __restrict__ r,
+                        const double* __restrict__ d, double theta, double theta_d, double* __restrict__ r,
                         double* __restrict__ t, long long n) {
   for (long long i = threadIdx.x + (long long)blockIdx.x * blockDim.x; i < n;
        i += (long long)blockDim.x * gridDim.x) {
     double rv = hx[i] - theta * x[i];
-    double den = theta - d[i];
+    double den = theta_d - d[i];
     if (fabs(den) < 1e-12) den = den < 0 ? -1e-12 : 1e-12;
     r[i] = rv;
     t[i] = rv / den;
@@ -214,9 +214,9 @@ void launch_scale(double a, double* y, long long n, cudaStream_t st) {
 void launch_add_const(double a, double* y, long long n, cudaStream_t st) {
   k_add_const<<<grid_for(n), 256, 0, st>>>(a, y, n);
 }
-void launch_residual_precond(const double* x, const double* hx, const double* d, double theta,
+void launch_residual_precond(const double* x, const double* hx, const double* d, double theta, double theta_d,
                              double* r, double* t, long long n, cudaStream_t st) {
-  k_resid<<<grid_for(n), 256, 0, st>>>(x, hx, d, theta, r, t, n);
+  k_resid<<<grid_for(n), 256, 0, st>>>(x, hx, d, theta, theta_d, r, t, n);
 }
 void launch_diag(const PsiBlockDev* blocks, int nblocks, const DiagTask* tasks, const int* task_begin,
                  double* out_p, cudaStream_t st) {

@@ -44,8 +44,10 @@ void launch_project_out(const double* V, long long ldv, const double* c, int m, 
 void launch_add_const(double a, double* y, long long n, cudaStream_t st);
 // y = a * y
 void launch_scale(double a, double* y, long long n, cudaStream_t st);
-// t = r / clamp(theta - d)   with |theta - d| >= 1e-12, sign kept; r = hx - theta*x computed on the fly
-void launch_residual_precond(const double* x, const double* hx, const double* d, double theta,
+// r = hx - theta*x ; t = r / clamp(theta_d - d) with |theta_d - d| >= 1e-12, sign kept.  theta is the Ritz value of
+// the operator hx was made with (e_core included), theta_d the same value on the scale of the diagonal d
+// (which is stored without e_core).
+void launch_residual_precond(const double* x, const double* hx, const double* d, double theta, double theta_d,
                              double* r, double* t, long long n, cudaStream_t st);
 // diag(H_eff): out_p[block] = sum_tasks alpha * diag(L) (x) diag(R)
 void launch_diag(const PsiBlockDev* blocks, int nblocks, const DiagTask* tasks, const int* task_begin,

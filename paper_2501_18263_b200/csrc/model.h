@@ -140,6 +140,9 @@ struct dmrg_ctx {
     return b;
   }
   void invalidate_site(int i) {     // site tensor i changed
+    if (k > 0 && (i <= k - 1 || i >= k + 2)) {   // it lies inside a block of the prepared problem: that problem is gone
+      k = 0; left.reset(); right.reset(); apply_plan.clear();
+    }
     for (auto it = left_cache.begin(); it != left_cache.end();) it = it->first >= i ? left_cache.erase(it) : std::next(it);
     for (auto it = right_cache.begin(); it != right_cache.end();) it = it->first <= i ? right_cache.erase(it) : std::next(it);
   }

@@ -158,6 +158,26 @@ Planner::HOut& Planner::p2_out(HChunk& ch, const Item& it, int b0, int cnt, int 
 void Planner::add_piece(const Item& it, int b0, int cnt) {
   if (chunks_.empty()) chunks_.emplace_back();
   const bool batched = it.strideC != 0;
+  if (batched) {
+    // Batched outputs of one chunk must be identical or disjoint: each becomes its own list of output tiles, and two
+    // lists that overlap would read-modify-write the same C tiles from different CTAs of one launch.  The callers'
+    // runs are disjoint-or-identical, but the workspace split of Planner::add cuts different items at different
+    // places; a piece that overlaps an output of the current chunk without being equal to it opens a new chunk
+    // (phase 2 of consecutive chunks runs in order).
+    const double* lo = it.C + (long long)b0 * it.strideC;
+    const double* hi = lo + (long long)cnt * it.strideC;
+    auto conflict = [&](const HChunk& ch) {
+      auto f = ch.batched_out.lower_bound(lo);
+      if (f != ch.batched_out.begin()) {
+        auto pv = std::prev(f);
+        if (pv->second > lo) return true;                       // starts earlier, reaches into [lo, hi)
+      }
+      if (f != ch.batched_out.end() && f->first < hi && !(f->first == lo && f->second == hi)) return true;
+      return false;
+    };
+    if (conflict(chunks_.back())) chunks_.emplace_back();
+    chunks_.back().batched_out[lo] = hi;
+  }
   auto mkseg = [](const double* A, int lda, bool ta, const double* B, int ldb, bool tb, int K) {
     HSeg h{};
     h.s.A = A; h.s.B = B; h.s.lda = lda; h.s.ldb = ldb; h.s.K = K; h.s.count = 1;
@@ -205,8 +225,9 @@ void Planner::add_piece(const Item& it, int b0, int cnt) {
   if (!shared && chunks_.back().ws_used + zsz * cnt > cap_) chunks_.emplace_back();
   HChunk& ch = chunks_.back();
   const long long zoff = shared ? zoff_shared : ch.ws_used;
-  const bool mergeM = cnt > 1 && A1.stride != 0 && B1.stride == 0;
-  const bool mergeN = cnt > 1 && A1.stride == 0 && B1.stride != 0;
+  // (the kernel divides a stacked row index x < cnt * zr by zr with one umulhi, exact for x * zr < 2^32)
+  const bool mergeM = cnt > 1 && A1.stride != 0 && B1.stride == 0 && (unsigned long long)cnt * zr * zr < (1ull << 32);
+  const bool mergeN = cnt > 1 && A1.stride == 0 && B1.stride != 0 && (unsigned long long)cnt * zc * zc < (1ull << 32);
   const long long zld = mergeN ? (long long)cnt * zc : zc;       // leading dimension of Z
   const long long zstep = mergeN ? zc : zsz;                      // offset of Z[b] relative to Z[0]
   if (shared) {

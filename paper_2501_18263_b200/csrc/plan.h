@@ -115,6 +115,7 @@ class Planner {
     std::vector<HOut> p1;
     std::vector<HOut> p2;
     std::map<std::tuple<const double*, int, long long>, int> p2_index;  // (C, batch, strideC) -> p2 slot
+    std::map<const double*, const double*> batched_out;   // [begin, end) of the batched outputs of this chunk
     long long ws_used = 0;
   };
   void add_piece(const Item& it, int b0, int cnt);

@@ -10,15 +10,16 @@ namespace su2 {
 
 namespace {
 
-long double fact(int n) {   // n! for 0 <= n <= 80
-  static long double t[81];
-  static bool init = false;
-  if (!init) {
+struct FactTable {
+  long double t[81];
+  FactTable() {
     t[0] = 1.0L;
     for (int i = 1; i <= 80; ++i) t[i] = t[i - 1] * (long double)i;
-    init = true;
   }
-  return (n < 0 || n > 80) ? 0.0L : t[n];
+};
+long double fact(int n) {   // n! for 0 <= n <= 80
+  static const FactTable tab;   // function-local static: initialised once, thread-safe (C++11)
+  return (n < 0 || n > 80) ? 0.0L : tab.t[n];
 }
 inline long double fh(int twice) { return fact(twice / 2); }   // (twice/2)!
 
