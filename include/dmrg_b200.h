@@ -207,7 +207,9 @@ int dmrg_env_export(dmrg_ctx* ctx, int32_t side, int32_t kind, int32_t i, int32_
  * dmrg_env_export are too large: BASELINE configs 3 and 4).  U(1)xU(1) contexts: `kind` as in dmrg_env_export and
  * `d2S` is ignored.  SU(2) contexts: kind 0 H, 1 C (rank 1/2), 2 A^0, 3 A^1, 4 B^0, 5 B^1, 6 S~ (rank 1/2) — the reduced
  * elements X_red[S',S] of <S'M'|X^k_q|SM> = <S M; k q|S' M'> X_red[S',S] — and d2S = 2S' - 2S selects the
- * class.  The block is chosen by the label of its INPUT sector, (q_up, q_dn) resp. (N, 2S), in the convention of
+ * class.  side: 0 / 1 = the left / right block of the prepared problem; 2 = the cached left block of sites 1..k-2,
+ * 3 = the cached right block of sites k+3..L (the predecessors of one blocking step; DMRG_ERR_ARG if the
+ * environment cache no longer holds them on the device).  The block is chosen by the label of its INPUT sector, (q_up, q_dn) resp. (N, 2S), in the convention of
  * dmrg_psi_block: left block = content of the block, right block = label of the bond (electrons LEFT of it).
  * Returns *nops, *rows (output sector), *cols (input sector) and, if h_out != NULL, the nops x rows x cols
  * row-major array; *rows = *cols = 0 if the class has no block with that input sector.  Operator order inside a

@@ -782,8 +782,17 @@ int dmrg_env_export(dmrg_ctx* ctx, int32_t side, int32_t kind, int32_t i, int32_
 int dmrg_env_export_block(dmrg_ctx* ctx, int32_t side, int32_t kind, int32_t d2S, int32_t qa, int32_t qb, int32_t* nops,
                           int32_t* rows, int32_t* cols, double* h_out) {
   API_BEGIN
-  DMRG_REQUIRE(ctx->k > 0 && (side == 0 || side == 1) && nops && rows && cols, DMRG_ERR_ARG, "env_export_block: bad arguments");
-  const BlockSide& B = side == 0 ? *ctx->left : *ctx->right;
+  DMRG_REQUIRE(ctx->k > 0 && side >= 0 && side <= 3 && nops && rows && cols, DMRG_ERR_ARG, "env_export_block: bad arguments");
+  const BlockSide* Bp = side == 0 ? ctx->left.get() : side == 1 ? ctx->right.get() : nullptr;
+  if (side >= 2) {
+    auto& cache = side == 2 ? ctx->left_cache : ctx->right_cache;
+    auto f = cache.find(side == 2 ? ctx->k - 2 : ctx->k + 3);
+    DMRG_REQUIRE(f != cache.end() && !f->second->spilled, DMRG_ERR_ARG,
+                 "env_export_block: the predecessor block is not in the device tier of the environment cache");
+    Bp = f->second.get();
+    side -= 2;
+  }
+  const BlockSide& B = *Bp;
   const OpClass* C = nullptr;
   int ca = qa, cb = qb;     // the block's own content
   if (ctx->su2()) {
