@@ -75,8 +75,20 @@ def test_config3_u1_d4096_properties():
     """The configuration `bench.py` times by default (north_star target)."""
     d = _ctx(3)
     assert d.psi_size() == 8085937
-    _properties(d, 4, 2)
+    hx = _properties(d, 4, 2)
     d.close()
+    # the mbarrier pipeline and the worker streams leave no trace in the result: the same plan with every launch
+    # in order on one stream gives the same bits (compute-sanitizer is not available on this pool)
+    os.environ["DMRG_B200_SERIAL"] = "1"
+    try:
+        d2 = _ctx(3)
+    finally:
+        del os.environ["DMRG_B200_SERIAL"]
+    import torch
+    g = torch.Generator(device="cpu").manual_seed(2)
+    x = torch.randn(d2.psi_size(), dtype=torch.float64, generator=g).cuda()
+    assert torch.equal(d2.heff_apply(x), hx)
+    d2.close()
 
 
 def test_config3_su2_1024_multiplets_properties():

@@ -51,7 +51,7 @@ def _offsets(pb):
     return off
 
 
-def lean_parity(d, T, V, mps, v, got_flat, idxs, group_elems=60000):
+def lean_parity(d, T, V, mps, v, got_flat, idxs, group_elems=60000, keep_refs=False):
     """Compares the library's psi' blocks `idxs` with the lean oracle fed by exported operator blocks.
     Blocks are processed in groups (bounded export size).  Returns list of (idx, dL, dR, rel-L2, rel-max)."""
     pb = inputs.psi_blocks(mps)
@@ -67,7 +67,7 @@ def lean_parity(d, T, V, mps, v, got_flat, idxs, group_elems=60000):
         cur.append(i); acc += sz
     if cur:
         groups.append(cur)
-    res = []
+    res, refs = [], {}
     for g in groups:
         qL = {pb[i][0] for i in g}
         qR = {odmrg.qsub(N, pb[i][3]) for i in g}
@@ -77,8 +77,10 @@ def lean_parity(d, T, V, mps, v, got_flat, idxs, group_elems=60000):
             dL, dR = pb[i][4], pb[i][5]
             got = got_flat[off[i]:off[i] + dL * dR].reshape(dL, dR)
             res.append((i, dL, dR) + rel_block_errors(got, ref[i]))
+            if keep_refs:
+                refs[i] = ref[i]
         del lo, ref
-    return res, Ls.bytes + Rs.bytes
+    return res, Ls.bytes + Rs.bytes, refs
 
 
 def test_lean_machinery_against_the_full_oracle_config1():
@@ -90,7 +92,7 @@ def test_lean_machinery_against_the_full_oracle_config1():
     got = d.heff_apply(torch.from_numpy(v).cuda()).cpu().numpy()
     pb = inputs.psi_blocks(mps)
     idxs = choose_blocks(pb, 10, seed=1)
-    res, _ = lean_parity(d, T, V, mps, v, got, idxs, group_elems=2000)
+    res, _, _ = lean_parity(d, T, V, mps, v, got, idxs, group_elems=2000)
     d.close()
     for i, dL, dR, r2, rmax in res:
         assert r2 <= TOL and rmax <= 10 * TOL, (i, dL, dR, r2, rmax)
@@ -117,10 +119,10 @@ def test_config3_u1_d4096_sampled_blocks_against_the_oracle(config3):
     T, V, mps, v, d, got = config3
     pb = inputs.psi_blocks(mps)
     assert len(got) == 8085937
-    idxs = choose_blocks(pb, 12, seed=3, max_elems=20000)
-    assert len(idxs) >= 20
+    idxs = choose_blocks(pb, 30, seed=3, max_elems=30000)
+    assert len(idxs) >= 30
     t0 = time.time()
-    res, nbytes = lean_parity(d, T, V, mps, v, got, idxs)
+    res, nbytes, _ = lean_parity(d, T, V, mps, v, got, idxs)
     print("config 3: %d blocks, %.1f GB of operator blocks exported, %.0f s" % (len(res), nbytes / 1e9, time.time() - t0))
     for i, dL, dR, r2, rmax in res:
         print("  block %4d  %3d x %3d  rel-L2 %.2e  max %.2e" % (i, dL, dR, r2, rmax))
