@@ -150,3 +150,146 @@ def rel_block_errors(got, ref):
     """(rel-L2, max-abs / max-abs(ref)) of one block."""
     nr = np.linalg.norm(ref)
     return np.linalg.norm(got - ref) / nr, np.abs(got - ref).max() / np.abs(ref).max()
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# SU(2) contexts: reduced operator blocks -> U(1) operator blocks on the CG-expanded basis (oracle/su2.expand_mps)
+# ---------------------------------------------------------------------------------------------------------------
+SU2_KINDS = {"H": 0, "C": 1, "A0": 2, "A1": 3, "B0": 4, "B1": 5, "S": 6}
+SU2_K2 = {"H": 0, "C": 1, "A0": 0, "A1": 2, "B0": 0, "B1": 2, "S": 1}       # doubled rank
+SU2_DN = {"H": 0, "C": 1, "A0": 2, "A1": 2, "B0": 0, "B1": 0, "S": -1}      # particle-number change
+_R2 = 0.5 ** 0.5
+
+
+class ExportedSideSU2:
+    """Same interface as ExportedSide for an SU(2) context: the carried operators are irreducible tensor operators
+    stored by reduced elements, <S'M'|X^k_q|SM> = <S M; k q|S' M'> X_red[S',S] (include/dmrg_b200.h, DESIGN.md §9:
+    C_{+1/2} = a+_up, A^1_{+1} = a+_iu a+_ju (i<j), A^0 = (a+_iu a+_jd - a+_id a+_ju)/sqrt2 (i<=j), B^1_{+1} = -a+_iu a_jd,
+    B^0 = (a+_iu a_ju + a+_id a_jd)/sqrt2, S~_{+1/2} = -S_{x,dn}).  `block` expands the needed components with the
+    oracle's Clebsch-Gordan coefficients into U(1) operator blocks on the basis oracle/su2.expand_mps defines:
+    inside the U(1) sector (n_up, n_dn) the multiplets (N, S) with S >= |S_z| follow each other (`layout`)."""
+
+    def __init__(self, d, side, orbs, layout, N_tot):
+        """layout: dict U(1) bond label -> (dim, [((N_label, 2S), offset), ...]) of the block's open bond."""
+        from oracle import su2 as osu2
+        self.cg = osu2.cg
+        self.d, self.side = d, side
+        self.left = side in (0, 2)
+        self.orbs = list(orbs)
+        self.N_tot = N_tot
+        n2 = N_tot // 2
+        self.N = (n2, n2)
+        self.layout = {}
+        for lab, (dim, lay) in layout.items():
+            qc = lab if self.left else (n2 - lab[0], n2 - lab[1])
+            self.layout[qc] = (dim, lay)
+        self.sectors = {q: v[0] for q, v in self.layout.items()}
+        self.bytes = 0
+        self._cache = {}
+
+    def _fetch(self, kind, d2S, lab_in):
+        key = (kind, d2S, lab_in)
+        if key not in self._cache:
+            a = self.d.env_export_block(self.side, SU2_KINDS[kind], lab_in, d2S=d2S)
+            if a is not None:
+                self.bytes += a.nbytes
+            self._cache[key] = a
+        return self._cache[key]
+
+    def _component(self, kind, q2, qo, qi):
+        """(nops, D_out, D_in) array of the component q2 of every operator of `kind` between the U(1) content sectors."""
+        k2, dN = SU2_K2[kind], SU2_DN[kind]
+        Do, lay_o = self.layout[qo]
+        Di, lay_i = self.layout[qi]
+        Mi, Mo = qi[0] - qi[1], qo[0] - qo[1]
+        assert Mo - Mi == q2 and (qo[0] + qo[1]) - (qi[0] + qi[1]) == dN
+        off_o = {lab: off for lab, off in lay_o}
+        out = None
+        for (Nl, Si), oi in lay_i:
+            for d2S in range(-k2, k2 + 1, 2):
+                So = Si + d2S
+                lab_o = (Nl + dN if self.left else Nl - dN, So)
+                if So < 0 or lab_o not in off_o:
+                    continue
+                c = self.cg(Si, Mi, k2, q2, So, Mo)
+                if c == 0.0:
+                    continue
+                red = self._fetch(kind, d2S, (Nl, Si))
+                if red is None:
+                    continue
+                if out is None:
+                    out = np.zeros((red.shape[0], Do, Di))
+                oo = off_o[lab_o]
+                out[:, oo:oo + red.shape[1], oi:oi + red.shape[2]] += c * red
+        return out
+
+    def block(self, keep_q, L, want=("H", "C", "A", "B", "S"), s_orbs=None):
+        lo = self.orbs[0] if self.orbs else 0
+        n = len(self.orbs)
+        blk = odmrg.Block(self.orbs, self.sectors)
+        ops = blk.ops
+        comp_cache = {}
+
+        def comp(kind, q2, qo, qi):
+            key = (kind, q2, qo, qi)
+            if key not in comp_cache:
+                comp_cache[key] = self._component(kind, q2, qo, qi)
+            return comp_cache[key]
+
+        def pairs(du, dd):
+            out = set()
+            for q in keep_q:
+                out.add(((q[0] + du, q[1] + dd), q))
+                out.add((q, (q[0] - du, q[1] - dd)))
+            return [(qo, qi) for qo, qi in out if qo in self.sectors and qi in self.sectors]
+
+        def put(name, du, dd, comps):
+            """comps: list of (kind, q2, idx, coef)"""
+            op = ops.setdefault(name, BlockOp())
+            for qo, qi in pairs(du, dd):
+                m = None
+                for kind, q2, idx, coef in comps:
+                    a = comp(kind, q2, qo, qi)
+                    if a is None:
+                        continue
+                    m = coef * a[idx] if m is None else m + coef * a[idx]
+                if m is not None:
+                    op[(qo, qi)] = m
+
+        tri = lambda a, b: a * n - a * (a + 1) // 2 + (b - a - 1)        # a < b
+        tri0 = lambda a, b: a * n - a * (a - 1) // 2 + (b - a)           # a <= b
+        if "H" in want:
+            put("H", 0, 0, [("H", 0, 0, 1.0)])
+        if "C" in want:
+            for a in range(n):
+                put(("C", 2 * (lo + a)), 1, 0, [("C", 1, a, 1.0)])
+                put(("C", 2 * (lo + a) + 1), 0, 1, [("C", -1, a, 1.0)])
+        if "A" in want:
+            for a in range(n):
+                for b in range(a, n):
+                    i, j = lo + a, lo + b
+                    if a < b:
+                        put(("A", 2 * i, 2 * j), 2, 0, [("A1", 2, tri(a, b), 1.0)])
+                        put(("A", 2 * i + 1, 2 * j + 1), 0, 2, [("A1", -2, tri(a, b), 1.0)])
+                        put(("A", 2 * i, 2 * j + 1), 1, 1, [("A1", 0, tri(a, b), _R2), ("A0", 0, tri0(a, b), _R2)])
+                        put(("A", 2 * i + 1, 2 * j), 1, 1, [("A1", 0, tri(a, b), _R2), ("A0", 0, tri0(a, b), -_R2)])
+                    else:
+                        put(("A", 2 * i, 2 * i + 1), 1, 1, [("A0", 0, tri0(a, a), _R2)])
+        if "B" in want:
+            for a in range(n):
+                for b in range(n):
+                    i, j, ix = lo + a, lo + b, a * n + b
+                    put(("B", 2 * i, 2 * j), 0, 0, [("B1", 0, ix, _R2), ("B0", 0, ix, _R2)])
+                    put(("B", 2 * i + 1, 2 * j + 1), 0, 0, [("B1", 0, ix, -_R2), ("B0", 0, ix, _R2)])
+                    put(("B", 2 * i, 2 * j + 1), 1, -1, [("B1", 2, ix, -1.0)])
+                    put(("B", 2 * i + 1, 2 * j), -1, 1, [("B1", -2, ix, 1.0)])
+        if "S" in want:
+            ext = [x for x in range(L) if x not in self.orbs]
+            for idx, x in enumerate(ext):
+                if s_orbs is not None and x not in s_orbs:
+                    ops[("S", 2 * x)] = BlockOp(); ops[("S", 2 * x + 1)] = BlockOp()
+                    continue
+                put(("S", 2 * x), -1, 0, [("S", -1, idx, 1.0)])          # S_{x,up} = S~_{-1/2}
+                put(("S", 2 * x + 1), 0, -1, [("S", 1, idx, -1.0)])      # S_{x,dn} = -S~_{+1/2}
+        self._cache.clear()
+        return blk

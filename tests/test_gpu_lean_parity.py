@@ -36,11 +36,20 @@ def _ctx(T, V, mps, **kw):
     return d
 
 
-def _sides(d, mps):
-    N, k, L = (mps.n_up, mps.n_dn), mps.k, mps.L
-    Ls = ExportedSide(d, 0, range(0, k - 1), mps.sectors[k - 1], N)
-    Rs = ExportedSide(d, 1, range(k + 1, L), {odmrg.qsub(N, q): dim for q, dim in mps.sectors[k + 1].items()}, N)
-    return Ls, Rs
+def u1_side_factory(d, mps):
+    """mk(side code, orbitals, bond): the exported block whose open bond is `bond` (U(1)xU(1) context)."""
+    N = (mps.n_up, mps.n_dn)
+
+    def mk(code, orbs, bond):
+        sec = mps.sectors[bond] if code in (0, 2) else {odmrg.qsub(N, q): dim for q, dim in mps.sectors[bond].items()}
+        return ExportedSide(d, code, orbs, sec, N)
+    return mk
+
+
+def _sides(d, mps, mk=None):
+    k, L = mps.k, mps.L
+    mk = mk or u1_side_factory(d, mps)
+    return mk(0, range(0, k - 1), k - 1), mk(1, range(k + 1, L), k + 1)
 
 
 def _offsets(pb):
@@ -51,13 +60,14 @@ def _offsets(pb):
     return off
 
 
-def lean_parity(d, T, V, mps, v, got_flat, idxs, group_elems=60000, keep_refs=False):
+def lean_parity(d, T, V, mps, v, got_flat, idxs, group_elems=60000, keep_refs=False, mk=None):
     """Compares the library's psi' blocks `idxs` with the lean oracle fed by exported operator blocks.
-    Blocks are processed in groups (bounded export size).  Returns list of (idx, dL, dR, rel-L2, rel-max)."""
+    Blocks are processed in groups (bounded export size).  Returns list of (idx, dL, dR, rel-L2, rel-max); with
+    got_flat = None only the oracle's blocks are computed (keep_refs)."""
     pb = inputs.psi_blocks(mps)
     N, L = (mps.n_up, mps.n_dn), mps.L
     off = _offsets(pb)
-    Ls, Rs = _sides(d, mps)
+    Ls, Rs = _sides(d, mps, mk)
     order = sorted(idxs, key=lambda i: pb[i][4] * pb[i][5])
     groups, cur, acc = [], [], 0
     for i in order:
@@ -75,8 +85,9 @@ def lean_parity(d, T, V, mps, v, got_flat, idxs, group_elems=60000, keep_refs=Fa
         ref = lo.apply_blocks(v, g)
         for i in g:
             dL, dR = pb[i][4], pb[i][5]
-            got = got_flat[off[i]:off[i] + dL * dR].reshape(dL, dR)
-            res.append((i, dL, dR) + rel_block_errors(got, ref[i]))
+            if got_flat is not None:
+                got = got_flat[off[i]:off[i] + dL * dR].reshape(dL, dR)
+                res.append((i, dL, dR) + rel_block_errors(got, ref[i]))
             if keep_refs:
                 refs[i] = ref[i]
         del lo, ref
@@ -135,14 +146,14 @@ def test_config3_u1_d4096_sampled_blocks_against_the_oracle(config3):
     assert max(dL * dR for _, dL, dR, _, _ in res) == max(b[4] * b[5] for b in pb)
 
 
-def _check_definition(d, mps, side_obj, left, strings):
+def _check_definition(d, mps, side_obj, left, strings, nkeep=(2, 2), max_dim=10 ** 9):
     """Exported normal operators against <b'|o_1 o_2|b> evaluated from the MPS tensors (every exported sector)."""
     N = (mps.n_up, mps.n_dn)
     k, L = mps.k, mps.L
     sites = list(range(1, k)) if left else list(range(k + 2, L + 1))
     tensors = mps.left if left else mps.right
-    qs = sorted(side_obj.sectors, key=lambda q: -side_obj.sectors[q])
-    keep = set(qs[:2] + qs[len(qs) // 2:len(qs) // 2 + 2])      # the two largest sectors and two mid-sized ones
+    qs = sorted((q for q in side_obj.sectors if side_obj.sectors[q] <= max_dim), key=lambda q: -side_obj.sectors[q])
+    keep = set(qs[:nkeep[0]] + qs[len(qs) // 2:len(qs) // 2 + nkeep[1]])      # the largest sectors and mid-sized ones
     blk = side_obj.block(keep, L, want=("C", "A", "B"))
     worst, nchecked = 0.0, 0
     for name, string in strings:
@@ -208,21 +219,22 @@ def test_config3_exported_operators_against_their_definition(config3):
     assert w <= 1e-11
 
 
-def _one_step(d, T, V, mps, left, q_new, s_orbs):
+def _one_step(d, T, V, mps, left, q_new, s_orbs, mk=None):
     """H{q_new, q_new} and S_x{.., q_new} (x in s_orbs) of the current block from ONE oracle enlarge-and-project step
      applied to the exported predecessor block; compared with the exported current block."""
     N = (mps.n_up, mps.n_dn)
     k, L = mps.k, mps.L
     w = odmrg.w_from_V(V)
+    mk = mk or u1_side_factory(d, mps)
     if left:
         site = k - 1                                   # absorbed site (1-based); orbital k-2
-        old = ExportedSide(d, 2, range(0, k - 2), mps.sectors[k - 2], N)
-        new = ExportedSide(d, 0, range(0, k - 1), mps.sectors[k - 1], N)
+        old = mk(2, range(0, k - 2), k - 2)
+        new = mk(0, range(0, k - 1), k - 1)
         iso = {(qi, odmrg.SITE_Q[s]): A for (qi, s), A in mps.left[site].items()}
     else:
         site = k + 2                                   # orbital k+1
-        old = ExportedSide(d, 3, range(k + 2, L), {odmrg.qsub(N, q): dim for q, dim in mps.sectors[k + 2].items()}, N)
-        new = ExportedSide(d, 1, range(k + 1, L), {odmrg.qsub(N, q): dim for q, dim in mps.sectors[k + 1].items()}, N)
+        old = mk(3, range(k + 2, L), k + 2)
+        new = mk(1, range(k + 1, L), k + 1)
         iso = {}
         for (qi, s), Bm in mps.right[site].items():
             qo = odmrg.qadd(qi, odmrg.SITE_Q[s])
