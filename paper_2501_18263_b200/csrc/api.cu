@@ -366,9 +366,10 @@ static void cache_enforce(dmrg_ctx* ctx, int near, cudaStream_t st) {
   }
 }
 
-static void cache_put(dmrg_ctx* ctx, bool left, int key, const std::shared_ptr<BlockSide>& b, cudaStream_t st) {
+// `near`: the bond the caller is heading for (distances decide which cached block leaves the device first)
+static void cache_put(dmrg_ctx* ctx, bool left, int key, const std::shared_ptr<BlockSide>& b, cudaStream_t st, int near = -1) {
   (left ? ctx->left_cache : ctx->right_cache)[key] = b;
-  cache_enforce(ctx, key, st);
+  cache_enforce(ctx, near >= 0 ? near : key, st);
 }
 
 static void build_side(dmrg_ctx* ctx, bool left, int upto, cudaStream_t st, double* flops_last) {
@@ -392,7 +393,7 @@ static void build_side(dmrg_ctx* ctx, bool left, int upto, cudaStream_t st, doub
     std::shared_ptr<BlockSide> nb = su ? renormalize_block_su2(ctx, *blk, i, st, flops_last)
                                        : renormalize_block(ctx, *blk, i, st, flops_last);
     (left ? ctx->left : ctx->right) = nb;     // in use: the cache must not move it to the host tier
-    cache_put(ctx, left, i, nb, st);
+    cache_put(ctx, left, i, nb, st, upto);   // keep what is close to the bond being prepared, not to the step in progress
     return nb;
   };
   if (left) for (int i = from + 1; i <= upto; ++i) blk = step(i);

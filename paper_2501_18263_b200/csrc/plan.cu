@@ -7,7 +7,7 @@
 namespace dmrg {
 
 int Plan::launches() const {
-  int n = 0;
+  int n = fused.launches();
   for (const auto& c : chunks) n += c.p1.launches() + c.p2.launches();
   return n;
 }
@@ -44,8 +44,36 @@ void collect(const Phase& ph, std::vector<Launch>& v) {
 }
 }  // namespace
 
+// fused small-sector stage: the launches of the tile classes are independent (disjoint outputs)
+static void run_fused(const FusedPhase& f, cudaStream_t st, int64_t* launch_counter, Exec* ex) {
+  int nl = 0;
+  for (int c = 0; c < FUSED_NCLASSES; ++c) nl += f.nouts[c] > 0;
+  if (nl == 0) return;
+  if (launch_counter) *launch_counter += nl + (f.nred > 0);
+  if (!ex || nl == 1) {
+    for (int c = FUSED_NCLASSES - 1; c >= 0; --c)
+      DMRG_CUDA(launch_fused(c, f.outs.p, f.tasks.p, f.order[c].p, f.nouts[c], st));
+  } else {
+    DMRG_CUDA(cudaEventRecord(ex->fork, st));
+    const int nw = std::min<int>(Exec::NW, nl);
+    for (int i = 0; i < nw; ++i) DMRG_CUDA(cudaStreamWaitEvent(ex->w[i], ex->fork, 0));
+    int w = 0;
+    for (int c = FUSED_NCLASSES - 1; c >= 0; --c) {
+      if (f.nouts[c] <= 0) continue;
+      DMRG_CUDA(launch_fused(c, f.outs.p, f.tasks.p, f.order[c].p, f.nouts[c], ex->w[w % nw]));
+      ++w;
+    }
+    for (int i = 0; i < nw; ++i) {
+      DMRG_CUDA(cudaEventRecord(ex->join[i], ex->w[i]));
+      DMRG_CUDA(cudaStreamWaitEvent(st, ex->join[i], 0));
+    }
+  }
+  if (f.nred > 0) launch_reduce_partials(f.red.p, f.nred, 1, st);
+}
+
 void Plan::run(cudaStream_t st, int64_t* launch_counter, Exec* ex) const {
   const int n = (int)chunks.size();
+  run_fused(fused, st, launch_counter, ex);
   for (int stage = 0; stage <= n; ++stage) {
     std::vector<Launch> ls;
     if (stage > 0) collect(chunks[stage - 1].p2, ls);
@@ -87,6 +115,17 @@ void Plan::run_profiled(cudaStream_t st, std::vector<LaunchRecord>* out) const {
   };
   out->clear();
   mark();
+  for (int c = FUSED_NCLASSES - 1; c >= 0; --c) {     // phase 3 = fused small-sector kernel, shape = tile class
+    if (fused.nouts[c] <= 0) continue;
+    DMRG_CUDA(launch_fused(c, fused.outs.p, fused.tasks.p, fused.order[c].p, fused.nouts[c], st));
+    mark();
+    out->push_back(LaunchRecord{0, 3, c, fused.nouts[c], fused.cls_flops[c], 0.f});
+  }
+  if (fused.nred > 0) {
+    launch_reduce_partials(fused.red.p, fused.nred, 1, st);
+    mark();
+    out->push_back(LaunchRecord{0, 3, -1, fused.nred, 0.0, 0.f});
+  }
   for (size_t c = 0; c < chunks.size(); ++c)
     for (int p = 0; p < 2; ++p) {
       const Phase& ph = p == 0 ? chunks[c].p1 : chunks[c].p2;
@@ -124,6 +163,7 @@ void Planner::add(const Item& it) {
   DMRG_REQUIRE(it.count >= 1, DMRG_ERR_ARG, "planner: empty item");
   ++n_items_;
   n_products_ += it.count;
+  if (add_fused(it)) return;
   if (it.nmat == 2) {
     fa_ += item_flops(it);
     add_piece(it, 0, it.count);
@@ -138,6 +178,45 @@ void Planner::add(const Item& it) {
   DMRG_REQUIRE(zsz <= cap_, DMRG_ERR_ALLOC, "planner: workspace cap smaller than one intermediate block");
   int per = (int)std::min<long long>(it.count, cap_ / zsz);
   for (int b0 = 0; b0 < it.count; b0 += per) add_piece(it, b0, std::min(per, it.count - b0));
+}
+
+// Items whose every dimension fits one tile of the fused kernel (<= 64 after padding) and that accumulate into one
+// output (not a batch of outputs) join that output's task list; the intermediate X*Y never leaves the SM.
+bool Planner::add_fused(const Item& it) {
+  if (!fused_on_ || it.strideC != 0) return false;
+  const int DMAX = fused_max_, KMAX = fused_maxk_;
+  FTask t{};
+  int M, N;
+  if (it.nmat == 3) {
+    M = it.X.rows; N = it.W.cols;
+    if (N > FUSED_MAX_N || M > DMAX || N > DMAX || it.X.cols > KMAX || it.Y.cols > KMAX) return false;
+    t.A = it.X.p; t.rsA = it.X.stride; t.lda = it.X.ld;
+    t.P = it.Y.p; t.rsP = it.Y.stride; t.ldp = it.Y.ld;
+    t.B = it.W.p; t.rsB = it.W.stride; t.ldb = it.W.ld;
+    t.mi = (short)it.X.cols; t.ni = (short)it.Y.cols;
+    t.flags = (it.X.tr ? 1 : 0) | (it.Y.tr ? 2 : 0) | (it.W.tr ? 4 : 0);
+    fe_ += it.count * (fl(M, it.X.cols, it.Y.cols) + fl(M, it.Y.cols, N));
+  } else {
+    M = it.X.rows; N = it.Y.cols;
+    if (N > FUSED_MAX_N || M > DMAX || N > DMAX || it.X.cols > KMAX) return false;
+    t.A = nullptr; t.rsA = 0; t.lda = 0;
+    t.P = it.X.p; t.rsP = it.X.stride; t.ldp = it.X.ld;
+    t.B = it.Y.p; t.rsB = it.Y.stride; t.ldb = it.Y.ld;
+    t.mi = 0; t.ni = (short)it.X.cols;
+    t.flags = (it.X.tr ? 2 : 0) | (it.Y.tr ? 4 : 0);
+    fe_ += it.count * fl(M, it.X.cols, N);
+  }
+  t.count = it.count; t.alpha = it.alpha;
+  fa_ += item_flops(it);
+  auto f = fused_index_.find(it.C);
+  if (f == fused_index_.end()) {
+    f = fused_index_.emplace(it.C, (int)fused_.size()).first;
+    fused_.push_back(HFOut{it.C, it.ldc, M, N, {}});
+  }
+  HFOut& o = fused_[f->second];
+  DMRG_REQUIRE(o.M == M && o.N == N && o.ldc == it.ldc, DMRG_ERR_ARG, "planner: one output with two shapes");
+  o.tasks.push_back(t);
+  return true;
 }
 
 Planner::HOut& Planner::p2_out(HChunk& ch, const Item& it, int b0, int cnt, int M, int N) {
@@ -372,8 +451,121 @@ void Planner::finish(Plan* plan, cudaStream_t st) {
     hv.swap(ex);
     scratch_max = std::max(scratch_max, sc_used);
   }
+  // ---- fused small-sector outputs: tile class, split of heavy task lists into parts, launch order ----
+  struct FPart { int out; bool partial; long long sc_off; std::vector<FTask> tasks; double cost; int cls; };
+  std::vector<FPart> fparts;
+  struct FRed { int out; long long sc_off; int nparts; };
+  std::vector<FRed> freds;
+  long long fsc_used = 0;
+  {
+    // cost of one repeat for ONE strip (a warp): MACs + an overhead per task (descriptor, first-fragment latency)
+    auto unit_cost = [](const HFOut& o, const FTask& t, int rows) {
+      return rows * ((t.A ? (double)t.mi * t.ni : 0.0) + (double)t.ni * o.N) + 2048.0;
+    };
+    std::vector<int> cls(fused_.size());
+    std::vector<double> cost(fused_.size(), 0.0);
+    double cls_total[FUSED_NCLASSES] = {};
+    for (size_t i = 0; i < fused_.size(); ++i) {
+      const HFOut& o = fused_[i];
+      const int c = o.N / 8 - 1;
+      cls[i] = c;
+      const int rows = FUSED_STRIP;
+      for (auto& t : o.tasks) cost[i] += t.count * unit_cost(o, t, rows);
+      cls_total[c] += cost[i] * ((o.M + rows - 1) / rows);
+    }
+    for (size_t i = 0; i < fused_.size(); ++i) {
+      HFOut& o = fused_[i];
+      // aim at ~3 work items per resident warp of the class, all of about the same length
+      const int rows = FUSED_STRIP;
+      const double target = std::max(cls_total[cls[i]] / (148.0 * fused_warps_per_sm(cls[i]) * 3.0), 1.0);
+      long long units = 0;
+      for (auto& t : o.tasks) units += t.count;
+      int ns = (int)std::min<long long>(std::min<long long>((long long)std::ceil(cost[i] / target), 64), units);
+      if (ns < 1) ns = 1;
+      const long long mn = (long long)o.M * o.N;
+      if (ns > 1) { freds.push_back(FRed{(int)i, fsc_used, ns - 1}); }
+      const double per = cost[i] / ns;
+      size_t ti = 0; int rep = 0;
+      int made = 0;
+      for (int p = 0; p < ns; ++p) {
+        FPart part{(int)i, p > 0, p > 0 ? fsc_used + (long long)(p - 1) * mn : 0, {}, 0.0, cls[i]};
+        while (ti < o.tasks.size() && (p == ns - 1 || part.cost < per)) {
+          const FTask& t = o.tasks[ti];
+          const double uc = unit_cost(o, t, rows);
+          const int left = t.count - rep;
+          int take = left;
+          if (p != ns - 1) take = (int)std::min<double>(left, std::max(1.0, std::floor((per - part.cost) / uc + 0.5)));
+          FTask sub = t;
+          sub.count = take;
+          if (sub.A) sub.A += (long long)rep * t.rsA;
+          sub.P += (long long)rep * t.rsP;
+          sub.B += (long long)rep * t.rsB;
+          part.tasks.push_back(sub);
+          part.cost += take * uc;
+          rep += take;
+          if (rep >= t.count) { rep = 0; ++ti; }
+        }
+        if (!part.tasks.empty()) { fparts.push_back(std::move(part)); ++made; }
+      }
+      if (ns > 1) {
+        // parts that came out empty are at the end: the reduction folds only the partial tiles that were written
+        freds.back().nparts = std::max(0, made - 1);
+        fsc_used += (long long)(ns - 1) * mn;
+      }
+    }
+    scratch_max = std::max(scratch_max, fsc_used);
+  }
   if (scratch_max > 0) plan->scratch.allocate(al_, (size_t)scratch_max);
   double* sc = plan->scratch.p;
+  if (!fparts.empty()) {
+    FusedPhase& F = plan->fused;
+    std::vector<FOut> outs;
+    std::vector<FTask> tasks;
+    std::vector<std::pair<double, int>> ord[FUSED_NCLASSES];
+    for (auto& pt : fparts) {
+      const HFOut& o = fused_[pt.out];
+      FOut fo{};
+      fo.C = pt.partial ? sc + pt.sc_off : o.C;
+      fo.ldc = pt.partial ? o.N : o.ldc;
+      fo.M = o.M; fo.N = o.N;
+      fo.accumulate = pt.partial ? 0 : 1;
+      fo.task_begin = (int)tasks.size();
+      for (auto& t : pt.tasks) {
+        tasks.push_back(t);
+        F.cls_flops[pt.cls] += t.count * ((t.A ? fl(o.M, t.mi, t.ni) : 0.0) + fl(o.M, t.ni, o.N));
+      }
+      fo.task_end = (int)tasks.size();
+      ord[pt.cls].push_back({pt.cost, (int)outs.size()});
+      outs.push_back(fo);
+    }
+    for (int c = 0; c < FUSED_NCLASSES; ++c) {
+      std::stable_sort(ord[c].begin(), ord[c].end(), [](const std::pair<double, int>& a, const std::pair<double, int>& b) { return a.first > b.first; });
+      std::vector<int2> o;
+      for (auto& x : ord[c])
+        for (int r0 = 0; r0 < outs[x.second].M; r0 += FUSED_STRIP) o.push_back(make_int2(x.second, r0));
+      F.nouts[c] = (int)o.size();
+      if (!o.empty()) F.order[c].upload(al_, o, st);
+    }
+    F.ntasks = (int64_t)tasks.size();
+    F.outs.upload(al_, outs, st);
+    F.tasks.upload(al_, tasks, st);
+    std::vector<RedDesc> rd;
+    for (auto& r : freds) {
+      if (r.nparts <= 0) continue;
+      const HFOut& o = fused_[r.out];
+      RedDesc d{};
+      d.C = o.C; d.P = sc + r.sc_off; d.bsC = 0; d.M = o.M; d.N = o.N; d.ldc = o.ldc; d.nparts = r.nparts; d.batch = 1;
+      rd.push_back(d);
+    }
+    F.nred = (int)rd.size();
+    if (!rd.empty()) F.red.upload(al_, rd, st);
+    if (plan->print_stats)
+      for (int c = 0; c < FUSED_NCLASSES; ++c)
+        if (F.nouts[c])
+          fprintf(stderr, "plan fused N = %d: %d warps, flops %.4g\n", 8 * (c + 1), F.nouts[c], F.cls_flops[c]);
+  }
+  fused_.clear();
+  fused_index_.clear();
   auto build = [&](std::vector<HOut>& hv, Phase& ph, double* ws) {
     std::vector<GOut> outs;
     std::vector<GSeg> segs;

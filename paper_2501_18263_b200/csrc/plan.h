@@ -13,6 +13,7 @@
 #include <tuple>
 
 #include "common.h"
+#include "fused.cuh"
 #include "gemm.cuh"
 #include "kernels.cuh"
 
@@ -64,6 +65,22 @@ struct Chunk {
   Phase p1, p2;
 };
 
+// Outputs whose whole task list runs in the fused small-sector kernel (fused.cuh): one launch per tile class,
+// before the two-phase chunks (both accumulate into the same outputs, so the stages run one after the other).
+struct FusedPhase {
+  DevArray<FOut> outs;
+  DevArray<FTask> tasks;
+  DevArray<int2> order[FUSED_NCLASSES];     // (output, first row of the strip) work items of each class, heaviest first
+  int nouts[FUSED_NCLASSES] = {};           // number of work items (warps)
+  double cls_flops[FUSED_NCLASSES] = {};    // flops the launch of each class executes (padded dims)
+  DevArray<RedDesc> red;
+  int nred = 0;
+  int64_t ntasks = 0;
+  int launches() const { int n = nred > 0; for (int c = 0; c < FUSED_NCLASSES; ++c) n += nouts[c] > 0; return n; }
+  void clear() { outs.release(); tasks.release(); red.release(); nred = 0; ntasks = 0;
+                 for (int c = 0; c < FUSED_NCLASSES; ++c) { order[c].release(); nouts[c] = 0; cls_flops[c] = 0; } }
+};
+
 // Worker streams for running the independent launches of a plan stage concurrently (fork/join with
 // events around the caller's stream).  Kernels of different tile shapes have very different grid
 // sizes; run back to back each one ends in its own under-filled tail, run side by side they fill it.
@@ -81,6 +98,7 @@ struct LaunchRecord { int chunk, phase, shape, ntiles; double flops; float ms; }
 
 struct Plan {
   std::vector<Chunk> chunks;
+  FusedPhase fused;
   DevArray<double> workspace, scratch;
   bool print_stats = false;   // DMRG_B200_PLAN_STATS: per-shape tile fill printed when a plan is built
   long long ws_half = 0;   // elements per workspace half (two halves when there are several chunks)
@@ -94,7 +112,7 @@ struct Plan {
   void run(cudaStream_t st, int64_t* launch_counter, Exec* ex = nullptr) const;
   // Same launches, each bracketed by events (shape -1 = split-K reduction).  Synchronises `st`.
   void run_profiled(cudaStream_t st, std::vector<LaunchRecord>* out) const;
-  void clear() { chunks.clear(); workspace.release(); scratch.release(); }
+  void clear() { chunks.clear(); fused.clear(); workspace.release(); scratch.release(); }
 };
 
 class Planner {
@@ -119,6 +137,14 @@ class Planner {
     long long ws_used = 0;
   };
   void add_piece(const Item& it, int b0, int cnt);
+  bool add_fused(const Item& it);
+  struct HFOut { double* C; int ldc, M, N; std::vector<FTask> tasks; };
+  std::vector<HFOut> fused_;
+  std::map<const double*, int> fused_index_;
+  bool fused_on_ = std::getenv("DMRG_B200_NO_FUSED") == nullptr;
+  // largest output dimension / largest contraction extent routed to the fused kernel (measured: DESIGN.md §7)
+  int fused_max_ = std::getenv("DMRG_B200_FUSED_MAX") ? std::atoi(std::getenv("DMRG_B200_FUSED_MAX")) : 64;
+  int fused_maxk_ = std::getenv("DMRG_B200_FUSED_MAXK") ? std::atoi(std::getenv("DMRG_B200_FUSED_MAXK")) : 64;
   HOut& p2_out(HChunk& ch, const Item& it, int b0, int cnt, int M, int N);
   Allocator* al_;
   long long cap_;
