@@ -29,7 +29,6 @@ sys.path.insert(0, ROOT)
 
 METRIC = "heff_apply_fp64_gflops"
 UNIT = "GFLOP/s"
-SAMPLE_CFG = 1   # bounded CPU sample: BASELINE.json configs[1] (L=20, D=256)
 
 
 class ClockSampler:
@@ -81,73 +80,99 @@ class ClockSampler:
                 "reasons": sorted(reasons), "samples": len(sm)}
 
 
-def time_oracle_sample(steps, warmup):
-    """The CPU oracle on BASELINE.json configs[1]; GFLOP/s from the flops its own matmuls execute."""
-    from oracle import dmrg as odmrg
-    from paper_2501_18263_b200 import inputs
-    T, V, mps = inputs.make_config(SAMPLE_CFG)
-    pb = inputs.psi_blocks(mps)
-    orc = odmrg.TwoSiteOracle(T, V, mps.n_up, mps.n_dn, mps.k, mps.sectors, mps.left, mps.right, pb)
-    orc.build_env()
-    orc.terms()
-    v = inputs.make_psi0(mps, inputs.CONFIGS[SAMPLE_CFG]["seed"])
-    flops = oracle_apply_flops(orc)
-    for _ in range(warmup):
-        orc.apply(v)
-    t0 = time.perf_counter()
-    for _ in range(steps):
-        orc.apply(v)
-    dt = (time.perf_counter() - t0) / max(steps, 1)
+def _host_threads():
     try:
         import threadpoolctl
-        cores = max(p["num_threads"] for p in threadpoolctl.threadpool_info()) if threadpoolctl.threadpool_info() else os.cpu_count()
+        info = threadpoolctl.threadpool_info()
+        return int(max(p["num_threads"] for p in info)) if info else int(os.cpu_count())
     except Exception:
-        cores = os.cpu_count()
-    return {"value": flops / dt * 1e-9, "unit": UNIT, "cores": int(cores), "kind": "oracle",
-            "sample": "BASELINE configs[%d] (L=20, N=(10,10), D=256, middle bond): %d H_eff.psi, %.2f s each; "
-                      "flops = those of the oracle's own block matmuls" % (SAMPLE_CFG, steps, dt),
-            "ms_per_apply": dt * 1e3}
+        return int(os.cpu_count())
 
 
-def oracle_apply_flops(orc):
-    """Flops of the matmuls one oracle apply executes (instrumentation only: shapes, no arithmetic)."""
-    psi_keys = {}
-    for (qL, s1, s2, qRb, dL, dR) in orc.psi_blocks:
-        from oracle.dmrg import SITE_Q, qsub
-        psi_keys[((qL, SITE_Q[s1]), (SITE_Q[s2], qsub(orc.N, qRb)))] = (dL, dR)
-    by_left = {}
-    for (kl, kr), shp in psi_keys.items():
-        by_left.setdefault(kl, []).append((kr, shp))
-    fl = 0.0
-    for XL, XR, hc in orc.terms():
-        r_in, r_out = {}, {}
-        for (kro, kri), mR in XR.items():
-            r_in.setdefault(kri, []).append((kro, mR.shape))
-            r_out.setdefault(kro, []).append((kri, mR.shape))
-        for (klo, kli), mL in XL.items():
-            for kri, (dl, dr) in by_left.get(kli, ()):
-                for kro, shp in r_in.get(kri, ()):
-                    if (klo, kro) in psi_keys:
-                        fl += 2.0 * mL.shape[0] * mL.shape[1] * dr + 2.0 * mL.shape[0] * dr * shp[0]
-            if hc:
-                for kro, (dl, dr) in by_left.get(klo, ()):
-                    for kri, shp in r_out.get(kro, ()):
-                        if (kli, kri) in psi_keys:
-                            fl += 2.0 * mL.shape[1] * mL.shape[0] * dr + 2.0 * mL.shape[1] * dr * shp[1]
-    return fl
+def time_oracle_sample(d, T, V, mps, psi0, steps, warmup, nblocks=10, max_elems=9000):
+    """The CPU oracle (oracle/lean.py: the oracle's own formulas restricted to chosen output blocks) on a BOUNDED
+    sample of output blocks of the bench configuration, in the SAME analytic flop count as the GPU line: the flops
+    of a block are those of the library's task list for that block (dmrg_block_flops).
+
+    The oracle's block operators at this size cannot be built by the oracle itself in minutes (37 min at D = 4096),
+    so they are read from the library's environments (dmrg_env_export_block) BEFORE the timed region, exactly as in
+    tests/test_gpu_lean_parity.py, which checks them against the oracle; forming the complementary operators of the
+    sampled blocks is setup (the GPU's task-list build is not timed either).  Timed: the oracle's contraction loop
+    `_accumulate` (psi' blocks = sum over terms of mL psi mR^T) for the sampled blocks."""
+    import importlib.util
+    from oracle import dmrg as odmrg
+    from oracle import lean
+    from paper_2501_18263_b200 import inputs
+    spec = importlib.util.spec_from_file_location("lean_helpers", os.path.join(ROOT, "tests", "lean_helpers.py"))
+    lh = importlib.util.module_from_spec(spec)
+    spec.loader.exec_module(lh)
+    pb = inputs.psi_blocks(mps)
+    bf = d.block_flops()
+    N, k, L = (mps.n_up, mps.n_dn), mps.k, mps.L
+    # a fixed spread of block sizes: every 1/nblocks quantile of the blocks below max_elems, by analytic flops
+    cand = sorted((i for i in range(len(pb)) if 64 <= pb[i][4] * pb[i][5] <= max_elems), key=lambda i: bf[i])
+    if not cand:
+        cand = sorted(range(len(pb)), key=lambda i: bf[i])
+    idxs = sorted({cand[min(len(cand) - 1, int((q + 0.5) / nblocks * len(cand)))] for q in range(nblocks)})
+    Ls = lh.ExportedSide(d, 0, range(0, k - 1), mps.sectors[k - 1], N)
+    Rs = lh.ExportedSide(d, 1, range(k + 1, L), {odmrg.qsub(N, q): dim for q, dim in mps.sectors[k + 1].items()}, N)
+    qL = {pb[i][0] for i in idxs}
+    qR = {odmrg.qsub(N, pb[i][3]) for i in idxs}
+    orc = lean.LeanTwoSiteOracle(T, V, mps.n_up, mps.n_dn, k, pb, Ls.block(qL, L), Rs.block(qR, L))
+    psi = orc.unflatten(np.asarray(psi0, dtype=np.float64))
+    keys = [orc.block_key(i) for i in idxs]
+    terms = orc.terms({kk[0] for kk in keys}, {kk[1] for kk in keys})
+
+    def one_pass():
+        out = {kk: np.zeros_like(psi[kk]) for kk in keys}
+        orc._accumulate(terms, psi, out)
+        return out
+    for _ in range(warmup):
+        one_pass()
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        one_pass()
+    dt = (time.perf_counter() - t0) / max(steps, 1)
+    flops = float(sum(bf[i] for i in idxs))
+    return {"value": flops / dt * 1e-9, "unit": UNIT, "cores": _host_threads(), "kind": "oracle",
+            "sample": "the bench configuration itself: %d of its %d psi' output blocks (dims %s), %.3f %% of the analytic flops of one "
+                      "H_eff.psi, %.2f s of oracle time per pass; flops = the library's task-list count for those blocks "
+                      "(dmrg_block_flops), operator blocks exported from the library's environments before the timed region"
+                      % (len(idxs), len(pb), ", ".join("%dx%d" % (pb[i][4], pb[i][5]) for i in idxs),
+                         100.0 * flops / float(bf.sum()), dt),
+            "ms_per_apply": dt * 1e3, "sample_flops": flops, "apply_flops": float(bf.sum())}
+
+
+def _workload(cfg, mps, n_up, n_dn, su2, D):
+    return ("BASELINE configs[%d]: L=%d, N=(%d,%d), %s, D=%d%s, middle bond (%d,%d), one H_eff.psi per step"
+            % (cfg, mps.L, n_up, n_dn, "SU(2) S=0" if su2 else "U(1)xU(1)", D, " multiplets" if su2 else "", mps.k, mps.k + 1))
 
 
 def run_reference(args):
+    """`--impl reference`: the CPU oracle on the bench configuration (a bounded sample of its output blocks per step)."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    cb = time_oracle_sample(max(args.steps, 1), min(args.warmup, 1))
+    import torch
+    from paper_2501_18263_b200 import inputs
+    from paper_2501_18263_b200.binding import DMRG
+    cfg = args.config
+    if args.su2 or cfg == 4:
+        raise SystemExit("--impl reference: U(1)xU(1) configurations only")
+    c = inputs.CONFIGS[cfg]
+    D = args.D if args.D else c["D"]
+    T, V, mps = inputs.make_config(cfg, D=D)
+    psi0 = inputs.make_psi0(mps, c["seed"])
+    # the library only supplies the oracle's INPUTS here (the operator blocks of the two environments); see time_oracle_sample
+    d = DMRG(mps.L, mps.n_up, mps.n_dn, device=int(os.environ.get("LOCAL_RANK", "0")))
+    d.setup(T, V, mps)
+    cb = time_oracle_sample(d, T, V, mps, psi0, max(args.steps, 1), min(args.warmup, 3))
+    d.close()
     line = {"impl": "reference", "metric": METRIC, "value": cb["value"], "unit": UNIT, "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": cb["ms_per_apply"], "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": "BASELINE configs[3] H_eff.psi (L=40, N=(14,14), U(1)xU(1), D=4096, middle bond); the CPU "
-                                   "oracle cannot finish that size in minutes, so each step is a bounded sample of the "
-                                   "same path on the same input recipe: " + cb["sample"]},
+            "config": {"workload": _workload(cfg, mps, mps.n_up, mps.n_dn, False, D) + "; CPU oracle, each step a bounded "
+                                   "sample of that workload: " + cb["sample"]},
             "cpu_baseline": cb,
             "e2e": {"value": cb["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
     print(json.dumps(line))
@@ -195,6 +220,19 @@ def run_ours(args):
     x = torch.from_numpy(psi0).to(dev)
     y = torch.empty_like(x)
     peak_tf = d.fp64_peak()
+    dfma_tf = d.dfma_peak()
+    # cuBLAS DGEMM 8192^3 through torch: a yardstick for the FP64 tensor pipe, never on the product path
+    ga = torch.randn(8192, 8192, dtype=torch.float64, device=dev)
+    gb = torch.randn(8192, 8192, dtype=torch.float64, device=dev)
+    torch.matmul(ga, gb)
+    ge0, ge1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ge0.record()
+    for _ in range(3):
+        torch.matmul(ga, gb)
+    ge1.record()
+    torch.cuda.synchronize()
+    dgemm_tf = 3 * 2.0 * 8192.0 ** 3 / (ge0.elapsed_time(ge1) * 1e-3) * 1e-12
+    del ga, gb
     try:
         hbm_peak = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))["hbm_gbs"]
     except Exception:
@@ -239,7 +277,7 @@ def run_ours(args):
     _, rec = d.apply_profile(x, y)
     dom = {}
     for r in rec:
-        if r["shape"] == 8:
+        if r["shape"] == 8 and r["phase"] < 3:
             a = dom.setdefault(r["phase"], [0, 0.0, 0.0])
             a[0] += 1; a[1] += r["flops"]; a[2] += r["ms"]
     tot_ms = sum(r["ms"] for r in rec) or 1.0
@@ -247,7 +285,10 @@ def run_ours(args):
     per_shape = {}
     for r in rec:
         if 0 <= r["shape"] < 9 and r["flops"] > 0:
-            key = "%d:%dx%d" % (r["phase"], (32, 64, 128)[r["shape"] // 3], (32, 64, 128)[r["shape"] % 3])
+            if r["phase"] == 3:      # fused small-sector kernel: shape = N / 8 - 1 of the output blocks
+                key = "fused:N=%d" % (8 * (r["shape"] + 1))
+            else:
+                key = "%d:%dx%d" % (r["phase"], (32, 64, 128)[r["shape"] // 3], (32, 64, 128)[r["shape"] % 3])
             a = per_shape.setdefault(key, [0.0, 0.0])
             a[0] += r["ms"]; a[1] += r["flops"]
     per_shape = {k: [round(v[0], 3), round(v[1] / v[0] * 1e-9, 2)] for k, v in sorted(per_shape.items()) if v[0] > 0}
@@ -276,6 +317,11 @@ def run_ours(args):
         e2e_fl = job_flops / (e2e_max * 1e-3)
     e2e_val = e2e_fl * 1e-9
 
+    # the CPU oracle on a sample of this configuration's output blocks (needs the environments of THIS bond: before
+    # the renormalisation step below moves the context to the next one)
+    cpu_line = None
+    if rank == 0 and world == 1 and not args.no_cpu and not su2:
+        cpu_line = time_oracle_sample(d, T, V, mps, psi0, 2, 1)
     extra = {}
     if (rank == 0 or job_flops is not None) and not args.quick:    # sharded: Davidson runs in lock-step on all ranks
         # ---- Davidson: fixed 10 iterations from the random start vector
@@ -290,17 +336,17 @@ def run_ours(args):
         extra["davidson"] = {"iters": it, "ms_per_iter": (time.perf_counter() - t2) * 1e3 / it, "energy": E, "resid": rn}
         extra["env_build"] = {"setup_s": setup_s, "last_build_ms": st["last_build_ms"],
                               "last_renorm_step_gflop": st["flops_renorm"] * 1e-9}
-        if cfg <= 2 and not su2:
+        if cfg <= 3 and not su2 and job_flops is None:
             # BASELINE configs[2]: Davidson to 1e-8 and one operator-renormalisation step (site k joins the left block)
-            z2 = 0.01 * x
-            z2[int(torch.argmin(dg))] += 1.0
-            z2 /= torch.linalg.norm(z2)
-            t3 = time.perf_counter()
-            E2, it2, rn2 = d.davidson(z2, tol=1e-8, max_iter=400, max_basis=20)
-            torch.cuda.synchronize()
-            extra["davidson_1e-8"] = {"iters": it2, "ms_total": (time.perf_counter() - t3) * 1e3, "energy": E2, "resid": rn2}
-            nxt = inputs.make_mps(mps.L, n_up, n_dn, D, mps.k + 1, c["seed"], sectors=mps.sectors)
-            d.mps_set_site(mps.k, 0, nxt.left[mps.k])
+            if cfg <= 2:
+                z2 = 0.01 * x
+                z2[int(torch.argmin(dg))] += 1.0
+                z2 /= torch.linalg.norm(z2)
+                t3 = time.perf_counter()
+                E2, it2, rn2 = d.davidson(z2, tol=1e-8, max_iter=400, max_basis=20)
+                torch.cuda.synchronize()
+                extra["davidson_1e-8"] = {"iters": it2, "ms_total": (time.perf_counter() - t3) * 1e3, "energy": E2, "resid": rn2}
+            d.mps_set_site(mps.k, 0, inputs.make_left_site(mps.sectors, mps.k, c["seed"]))
             d.renormalize(0)
             torch.cuda.synchronize()
             s2 = d.stats()
@@ -308,14 +354,17 @@ def run_ours(args):
                                          "tflops": s2["flops_renorm"] / (s2["renorm_ms"] * 1e-3) * 1e-12,
                                          "includes": "host planning of the step + all launches + sync"}
 
-    # DRAM bytes per launch of the dominant kernel from the committed ncu --set full capture of this workload
-    # (profiles/r01_gemm128_full.md: dram__bytes_read.sum + dram__bytes_write.sum); only known for the default config.
+    # DRAM bytes per launch of the dominant kernel: written next to the committed ncu --set full summary of this
+    # workload (profiles/gemm128_traffic.json, dram__bytes_read.sum + dram__bytes_write.sum); default config only.
+    traffic_detail, traffic = None, None
     if cfg == 3 and not su2 and not args.D:
-        traffic_detail = {"phase1_bytes_per_launch": [26.02e9, 45.69e9], "phase2_bytes_per_launch": [28.67e9],
-                          "source": "profiles/r01_gemm128_full.md (three captured launches)"}
-        traffic = (26.02e9 + 45.69e9 + 28.67e9) / 3
-    else:
-        traffic_detail, traffic = None, None
+        try:
+            tj = json.load(open(os.path.join(ROOT, "profiles", "gemm128_traffic.json")))
+            per = [l["dram_read_bytes"] + l["dram_write_bytes"] for l in tj["launches"]]
+            traffic_detail = {"bytes_per_launch": per, "source": tj["source"]}
+            traffic = sum(per) / len(per)
+        except Exception:
+            pass
     if rank == 0:
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
                 "warmup": args.warmup, "ms_per_step": ms_max, "higher_is_better": True,
@@ -342,6 +391,10 @@ def run_ours(args):
                              "peak_source": "FP64 tensor-pipe (DMMA m8n8k4) register-only loop measured in this run "
                                             "(dmrg_fp64_peak) = 148 SM x 128 flop/clk x SM clock; MEASURED_PEAKS.json "
                                             "has no FP64 entry",
+                             "comparison_peaks": {"dmma_loop_tflops": peak_tf, "dfma_loop_tflops": dfma_tf,
+                                                  "cublas_dgemm_8192_tflops": dgemm_tf,
+                                                  "frac_of_dfma_loop": value / world * 1e-3 / dfma_tf,
+                                                  "frac_of_cublas_dgemm": value / world * 1e-3 / dgemm_tf},
                              "dominant_kernel": dict(dominant, achieved=(dom_fl / dom_ms * 1e-9 if dom_ms else None),
                                                      frac=(dom_fl / dom_ms * 1e-9 / peak_tf if dom_ms else None),
                                                      traffic=traffic_detail),
@@ -352,8 +405,8 @@ def run_ours(args):
                              "flops_executed_per_apply": st["flops_executed"]},
                 }
         line.update(extra)
-        if world == 1 and not args.no_cpu:
-            line["cpu_baseline"] = time_oracle_sample(2, 1)
+        if cpu_line is not None:
+            line["cpu_baseline"] = cpu_line
         print(json.dumps(line))
     d.close()
     if world > 1:

@@ -159,6 +159,11 @@ int dmrg_set_shard(dmrg_ctx* ctx, int32_t rank, int32_t count, dmrg_reduce_fn re
  * of the prepared problem; either pointer may be NULL. */
 int dmrg_shard_info(dmrg_ctx* ctx, int32_t* h_owner, double* h_flops);
 
+/* Analytic flops of one H_eff.psi per OUTPUT block of psi' (sum over the tasks that write the block of
+ * the cheaper contraction order on the unpadded dims); h_flops: nblocks doubles, their sum is dmrg_stats.flops_apply
+ * of an unsharded context.  Used to quote the CPU oracle's rate on a sample of blocks in the same flop count. */
+int dmrg_block_flops(dmrg_ctx* ctx, double* h_flops);
+
 /* Diagonal of H_eff in the psi layout. */
 int dmrg_heff_diag(dmrg_ctx* ctx, double* d_diag, void* stream);
 
@@ -228,6 +233,9 @@ int dmrg_su2_f_factor(int32_t twoSa, int32_t twoSk, int32_t twoSg, int32_t twokL
 /* Measured FP64 tensor-pipe (DMMA) peak of the device in TFLOP/s: a register-only mma loop on all
  * SMs, timed with CUDA events on `stream`. */
 int dmrg_fp64_peak(dmrg_ctx* ctx, double* h_tflops, void* stream);
+/* The same measurement with plain DFMA instructions (FP64 vector pipe) instead of DMMA: the second comparison peak of
+ * SURVEY.md 8(d). */
+int dmrg_dfma_peak(dmrg_ctx* ctx, double* h_tflops, void* stream);
 
 /* Per-launch timing of one H_eff.psi (measurement aid): runs dmrg_heff_apply with every
  * kernel launch of the task plan bracketed by CUDA events on `stream` and synchronises.  Up to `cap`

@@ -22,7 +22,7 @@ EXPORTS = [
     "dmrg_mps_set_site", "dmrg_env_build", "dmrg_renormalize", "dmrg_psi_layout", "dmrg_heff_apply",
     "dmrg_heff_diag", "dmrg_davidson", "dmrg_heff_apply_host", "dmrg_davidson_host", "dmrg_stats",
     "dmrg_env_export", "dmrg_fp64_peak", "dmrg_apply_profile", "dmrg_mps_set_site_su2", "dmrg_su2_f_factor",
-    "dmrg_mps_update_bond", "dmrg_set_shard", "dmrg_shard_info", "dmrg_env_export_block",
+    "dmrg_mps_update_bond", "dmrg_set_shard", "dmrg_shard_info", "dmrg_env_export_block", "dmrg_block_flops", "dmrg_dfma_peak",
 ]
 
 REDUCE_FN = C.CFUNCTYPE(C.c_int, C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p)
@@ -98,6 +98,8 @@ def load_library(build_if_missing: bool = True):
     lib.dmrg_env_export.argtypes = [vp, i32, i32, i32, i32, vp, C.POINTER(i64)]
     lib.dmrg_env_export_block.argtypes = [vp, i32, i32, i32, i32, i32, C.POINTER(i32), C.POINTER(i32), C.POINTER(i32), vp]
     lib.dmrg_fp64_peak.argtypes = [vp, dp, vp]
+    lib.dmrg_dfma_peak.argtypes = [vp, dp, vp]
+    lib.dmrg_block_flops.argtypes = [vp, vp]
     lib.dmrg_apply_profile.argtypes = [vp, vp, vp, i32, C.POINTER(LaunchInfo), C.POINTER(i32), vp]
     for name in EXPORTS:
         if name != "dmrg_last_error":
@@ -337,6 +339,17 @@ class DMRG:
         v = C.c_double()
         self._check(self.lib.dmrg_fp64_peak(self.ctx, C.byref(v), self._stream()))
         return v.value
+
+    def dfma_peak(self):
+        v = C.c_double()
+        self._check(self.lib.dmrg_dfma_peak(self.ctx, C.byref(v), self._stream()))
+        return v.value
+
+    def block_flops(self):
+        """Analytic flops of one H_eff.psi per output block (numpy array, psi_layout order)."""
+        out = np.zeros(len(self.psi_layout()[0]))
+        self._check(self.lib.dmrg_block_flops(self.ctx, _np_ptr(out)))
+        return out
 
     def apply_profile(self, psi_in, psi_out=None, cap=4096):
         """One H_eff.psi with per-launch event timing; returns (psi_out, list of dict per launch)."""

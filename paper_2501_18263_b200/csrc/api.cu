@@ -727,6 +727,13 @@ int dmrg_shard_info(dmrg_ctx* ctx, int32_t* h_owner, double* h_flops) {
   API_END
 }
 
+int dmrg_block_flops(dmrg_ctx* ctx, double* h_flops) {
+  API_BEGIN
+  DMRG_REQUIRE(ctx->k > 0 && h_flops && ctx->blk_flops.size() == ctx->psi.size(), DMRG_ERR_ARG, "block_flops: no problem prepared");
+  for (size_t i = 0; i < ctx->psi.size(); ++i) h_flops[i] = ctx->blk_flops[i];
+  API_END
+}
+
 int dmrg_stats(dmrg_ctx* ctx, dmrg_stats_t* out) {
   API_BEGIN
   DMRG_REQUIRE(out, DMRG_ERR_ARG, "stats: null pointer");
@@ -880,6 +887,16 @@ int dmrg_fp64_peak(dmrg_ctx* ctx, double* h_tflops, void* stream) {
   DevArray<double> scratch;
   scratch.allocate(&ctx->al, 64);
   DMRG_CUDA(measure_dmma_peak(scratch.p, h_tflops, (cudaStream_t)stream));
+  ctx->launches += 2;
+  API_END
+}
+
+int dmrg_dfma_peak(dmrg_ctx* ctx, double* h_tflops, void* stream) {
+  API_BEGIN
+  DMRG_REQUIRE(h_tflops, DMRG_ERR_ARG, "dfma_peak: null pointer");
+  DevArray<double> scratch;
+  scratch.allocate(&ctx->al, 64);
+  DMRG_CUDA(measure_dfma_peak(scratch.p, h_tflops, (cudaStream_t)stream));
   ctx->launches += 2;
   API_END
 }

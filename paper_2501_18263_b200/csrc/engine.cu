@@ -873,7 +873,7 @@ void prepare_superblock(dmrg_ctx* ctx, cudaStream_t st) {
   // from which every rank derives the same block -> rank map; pass 1 emits the items of the blocks this rank owns.
   std::vector<double> blk_flops(ctx->psi.size(), 0.0);
   for (int pass = ctx->shard_count > 1 ? 0 : 1; pass < 2; ++pass) {
-  if (pass == 1) assign_shard_owners(ctx, blk_flops);
+  if (pass == 1) { assign_shard_owners(ctx, blk_flops); ctx->blk_flops.assign(ctx->psi.size(), 0.0); }
   for (size_t bi = 0; bi < ctx->psi.size(); ++bi) {
     for (size_t gi = 0; gi < fgs.size(); ++gi) {
       const auto& f = fgs[gi];
@@ -940,6 +940,7 @@ void prepare_superblock(dmrg_ctx* ctx, cudaStream_t st) {
               it.Y = Mat{I.ptr(ib, 0), I.blocks[ib].cp, false, 0, in.dRp, in.dRp, in.dR, in.dR};
             }
             if (pass == 0) { blk_flops[fo->second] += item_flops(it); continue; }
+            ctx->blk_flops[fo->second] += item_flops(it);     // analytic flops per OUTPUT block (dmrg_block_flops)
             if (mine) planner.add(it);
             if (fo->second == (int)bi) {      // the diagonal is kept whole on every rank
               DiagTask d{};

@@ -179,6 +179,20 @@ __global__ void k_dmma_peak(double* out, int iters, double a, double b) {
   if (s == 12345.678) out[0] = s;   // keeps the loop alive without a store on the normal path
 }
 
+__global__ void k_dfma_peak(double* out, int iters, double a, double b) {
+  double c[16];
+#pragma unroll
+  for (int i = 0; i < 16; i++) c[i] = threadIdx.x + i;
+  for (int it = 0; it < iters; it++) {
+#pragma unroll
+    for (int i = 0; i < 16; i++) c[i] = fma(c[i], a, b);
+  }
+  double s = 0;
+#pragma unroll
+  for (int i = 0; i < 16; i++) s += c[i];
+  if (s == 12345.678) out[0] = s;
+}
+
 inline int grid_for(long long n) {
   long long g = (n + 255) / 256;
   return (int)(g < 1 ? 1 : (g > 1184 ? 1184 : g));
@@ -243,6 +257,26 @@ cudaError_t measure_dmma_peak(double* dummy, double* tflops, cudaStream_t st) {
   float ms = 0;
   cudaEventElapsedTime(&ms, e0, e1);
   double fl = 2.0 * 8 * 8 * 4 * 8.0 * iters * (threads / 32.0) * sms;
+  *tflops = fl / (ms * 1e-3) * 1e-12;
+  cudaEventDestroy(e0); cudaEventDestroy(e1);
+  return e;
+}
+
+cudaError_t measure_dfma_peak(double* dummy, double* tflops, cudaStream_t st) {
+  int dev = 0, sms = 0;
+  cudaGetDevice(&dev);
+  cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+  cudaEvent_t e0, e1;
+  cudaEventCreate(&e0); cudaEventCreate(&e1);
+  const int iters = 20000, threads = 1024;
+  k_dfma_peak<<<2 * sms, threads, 0, st>>>(dummy, 2000, 1.0000001, 1e-9);
+  cudaEventRecord(e0, st);
+  k_dfma_peak<<<2 * sms, threads, 0, st>>>(dummy, iters, 1.0000001, 1e-9);
+  cudaEventRecord(e1, st);
+  cudaError_t e = cudaEventSynchronize(e1);
+  float ms = 0;
+  cudaEventElapsedTime(&ms, e0, e1);
+  const double fl = 2.0 * 16.0 * iters * threads * 2.0 * sms;
   *tflops = fl / (ms * 1e-3) * 1e-12;
   cudaEventDestroy(e0); cudaEventDestroy(e1);
   return e;

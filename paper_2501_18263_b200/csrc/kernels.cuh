@@ -63,5 +63,7 @@ void launch_reduce_partials(const RedDesc* d, int n, int max_batch, cudaStream_t
 // register-only DMMA loop; returns achieved TFLOP/s
 constexpr int DIAG_MAX_DIM = 640;
 cudaError_t measure_dmma_peak(double* d_scratch, double* tflops, cudaStream_t st);
+// register-only DFMA loop (FP64 vector pipe); returns achieved TFLOP/s
+cudaError_t measure_dfma_peak(double* d_scratch, double* tflops, cudaStream_t st);
 
 }  // namespace dmrg

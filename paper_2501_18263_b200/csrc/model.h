@@ -162,6 +162,7 @@ struct dmrg_ctx {
   void* reduce_user = nullptr;
   std::vector<int> psi_owner;
   std::vector<double> shard_flops;               // analytic flops per rank of the prepared problem
+  std::vector<double> blk_flops;                 // analytic flops per output block of the prepared problem (all ranks' tasks)
   dmrg::Exec exec;                              // worker streams (plan.h)
   dmrg::Exec* ex() { return exec.ok ? &exec : nullptr; }
   dmrg_stats_t stats{};

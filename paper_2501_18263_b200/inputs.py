@@ -199,6 +199,29 @@ def make_mps(L: int, n_up: int, n_dn: int, D: int, k: int, seed: int, sectors=No
     return mps
 
 
+def make_left_site(sectors, i: int, seed: int):
+    """One random left-canonical site tensor (site i, bond i-1 -> bond i) by the recipe of make_mps, for a single
+    renormalisation step at a bond whose site tensors make_mps left open (sites k, k+1)."""
+    rng = np.random.Generator(np.random.PCG64(seed + 7919 + 31 * i))
+    site = {}
+    for qo in sorted(sectors[i]):
+        do = sectors[i][qo]
+        rows = []
+        for qi in sorted(sectors[i - 1]):
+            for s in range(4):
+                if _qadd(qi, s) == qo:
+                    rows.append((qi, s, sectors[i - 1][qi]))
+        nrow = sum(r[2] for r in rows)
+        assert nrow >= do, "sector clipping failed (left)"
+        Q, R = np.linalg.qr(rng.normal(size=(nrow, do)))
+        Q = Q * np.sign(np.diag(R))[None, :]
+        off = 0
+        for qi, s, d in rows:
+            site[(qi, s)] = np.ascontiguousarray(Q[off:off + d, :])
+            off += d
+    return site
+
+
 def psi_blocks(mps: MPSInput):
     """Ordered list of two-site wavefunction blocks (qL, s1, s2, qbond_R) with shapes.
 
