@@ -344,9 +344,10 @@ static void fetch_block(dmrg_ctx* ctx, BlockSide& b, cudaStream_t st) {
   ++ctx->n_fetches;
 }
 
-// Keeps the device-resident part of the cache under its cap: the resident block farthest from bond `near` goes to
-// the host tier, or is dropped when there is none (or it is full).  The blocks in use are never touched.
-static void cache_enforce(dmrg_ctx* ctx, int near, cudaStream_t st) {
+// Keeps the device-resident part of the cache under its cap: the resident block farthest from the two-site problem
+// at bond (kb, kb+1) the caller is heading for — left blocks measured from kb-1, right blocks from kb+2 — goes to the
+// host tier, or is dropped when there is none (or it is full).  The blocks in use are never touched.
+static void cache_enforce(dmrg_ctx* ctx, int kb, cudaStream_t st) {
   const uint64_t cap = env_cache_cap(ctx);
   while (true) {
     uint64_t res = 0;
@@ -357,7 +358,7 @@ static void cache_enforce(dmrg_ctx* ctx, int near, cudaStream_t st) {
         if (kv.second->spilled) continue;
         if (kv.second == ctx->left || kv.second == ctx->right) continue;    // in use: neither counted nor moved
         res += kv.second->bytes();
-        const int dist = std::abs(kv.first - near);
+        const int dist = std::abs(kv.first - (side == 0 ? kb - 1 : kb + 2));
         if (dist > far_dist) { far_dist = dist; far = kv.second; far_left = side == 0; far_key = kv.first; }
       }
     if (res <= cap || !far) return;
@@ -366,10 +367,10 @@ static void cache_enforce(dmrg_ctx* ctx, int near, cudaStream_t st) {
   }
 }
 
-// `near`: the bond the caller is heading for (distances decide which cached block leaves the device first)
-static void cache_put(dmrg_ctx* ctx, bool left, int key, const std::shared_ptr<BlockSide>& b, cudaStream_t st, int near = -1) {
+// kb: the bond the caller is heading for (distances decide which cached block leaves the device first)
+static void cache_put(dmrg_ctx* ctx, bool left, int key, const std::shared_ptr<BlockSide>& b, cudaStream_t st, int kb) {
   (left ? ctx->left_cache : ctx->right_cache)[key] = b;
-  cache_enforce(ctx, near >= 0 ? near : key, st);
+  cache_enforce(ctx, kb, st);
 }
 
 static void build_side(dmrg_ctx* ctx, bool left, int upto, cudaStream_t st, double* flops_last) {
@@ -387,13 +388,13 @@ static void build_side(dmrg_ctx* ctx, bool left, int upto, cudaStream_t st, doub
     // make room first: the block about to come back counts as needed
     fetch_block(ctx, *blk, st);
     (left ? ctx->left : ctx->right) = blk;
-    cache_enforce(ctx, upto, st);
+    cache_enforce(ctx, left ? upto + 1 : upto - 2, st);
   }
   auto step = [&](int i) {
     std::shared_ptr<BlockSide> nb = su ? renormalize_block_su2(ctx, *blk, i, st, flops_last)
                                        : renormalize_block(ctx, *blk, i, st, flops_last);
     (left ? ctx->left : ctx->right) = nb;     // in use: the cache must not move it to the host tier
-    cache_put(ctx, left, i, nb, st, upto);   // keep what is close to the bond being prepared, not to the step in progress
+    cache_put(ctx, left, i, nb, st, left ? upto + 1 : upto - 2);   // keep what is close to the bond being prepared
     return nb;
   };
   if (left) for (int i = from + 1; i <= upto; ++i) blk = step(i);
@@ -441,7 +442,7 @@ int dmrg_renormalize(dmrg_ctx* ctx, int32_t direction, void* stream) {
     DMRG_REQUIRE(k + 2 <= ctx->L, DMRG_ERR_ARG, "renormalize: already at the right end");
     auto r0 = std::chrono::steady_clock::now();
     ctx->left = ctx->su2() ? renormalize_block_su2(ctx, *ctx->left, k, st, &fl) : renormalize_block(ctx, *ctx->left, k, st, &fl);
-    cache_put(ctx, true, k, ctx->left, st);
+    cache_put(ctx, true, k, ctx->left, st, k + 1);
     ctx->stats.renorm_ms = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - r0).count();
     double f2 = 0;
     ctx->right.reset();
@@ -452,7 +453,7 @@ int dmrg_renormalize(dmrg_ctx* ctx, int32_t direction, void* stream) {
     auto r0 = std::chrono::steady_clock::now();
     ctx->right = ctx->su2() ? renormalize_block_su2(ctx, *ctx->right, k + 1, st, &fl)
                             : renormalize_block(ctx, *ctx->right, k + 1, st, &fl);
-    cache_put(ctx, false, k + 1, ctx->right, st);
+    cache_put(ctx, false, k + 1, ctx->right, st, k - 1);
     ctx->stats.renorm_ms = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - r0).count();
     double f2 = 0;
     ctx->left.reset();

@@ -21,7 +21,16 @@ void Exec::init() {
   DMRG_CUDA(cudaEventCreateWithFlags(&fork, cudaEventDisableTiming));
   ok = true;
 }
+cudaEvent_t Exec::event(size_t i) {
+  while (pool.size() <= i) {
+    cudaEvent_t e;
+    DMRG_CUDA(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+    pool.push_back(e);
+  }
+  return pool[i];
+}
 Exec::~Exec() {
+  for (auto e : pool) cudaEventDestroy(e);
   if (!ok) return;
   for (int i = 0; i < NW; ++i) { cudaStreamDestroy(w[i]); cudaEventDestroy(join[i]); }
   cudaEventDestroy(fork);
@@ -74,35 +83,58 @@ static void run_fused(const FusedPhase& f, cudaStream_t st, int64_t* launch_coun
 void Plan::run(cudaStream_t st, int64_t* launch_counter, Exec* ex) const {
   const int n = (int)chunks.size();
   run_fused(fused, st, launch_counter, ex);
-  for (int stage = 0; stage <= n; ++stage) {
-    std::vector<Launch> ls;
-    if (stage > 0) collect(chunks[stage - 1].p2, ls);
-    if (stage < n) collect(chunks[stage].p1, ls);
-    if (ls.empty()) continue;
-    if (launch_counter) *launch_counter += (int64_t)ls.size();
-    if (!ex || ls.size() == 1) {
-      for (auto& l : ls)
-        DMRG_CUDA(launch_shape(*l.ph, l.shape, st));
-    } else {
+  if (n == 0) return;
+  if (!ex) {
+    for (int c = 0; c < n; ++c)
+      for (int p = 0; p < 2; ++p) {
+        const Phase& ph = p ? chunks[c].p2 : chunks[c].p1;
+        std::vector<Launch> ls;
+        collect(ph, ls);
+        if (launch_counter) *launch_counter += (int64_t)ls.size() + (ph.nred > 0);
+        for (auto& l : ls) DMRG_CUDA(launch_shape(*l.ph, l.shape, st));
+        if (ph.nred > 0) launch_reduce_partials(ph.red.p, ph.nred, ph.red_max_batch, st);
+      }
+    return;
+  }
+  constexpr int LA = Exec::NW / 2, LB = Exec::NW - LA;        // streams of lane A (phase 1) / lane B (phase 2)
+  auto evA = [&](int c, int i) { return ex->event((size_t)c * (LA + LB + 1) + i); };
+  auto evB = [&](int c, int j) { return ex->event((size_t)c * (LA + LB + 1) + LA + j); };
+  auto evDone = [&](int c) { return ex->event((size_t)c * (LA + LB + 1) + LA + LB); };
+  DMRG_CUDA(cudaEventRecord(ex->fork, st));
+  for (int c = 0; c < n; ++c) {
+    // ---- lane A: phase 1 of chunk c ----
+    {
+      std::vector<Launch> ls;
+      collect(chunks[c].p1, ls);
       std::stable_sort(ls.begin(), ls.end(), [](const Launch& a, const Launch& b) { return a.work > b.work; });
-      DMRG_CUDA(cudaEventRecord(ex->fork, st));
-      const int nw = std::min<int>(Exec::NW, (int)ls.size());
-      for (int i = 0; i < nw; ++i) DMRG_CUDA(cudaStreamWaitEvent(ex->w[i], ex->fork, 0));
-      for (size_t i = 0; i < ls.size(); ++i) {
-        const Launch& l = ls[i];
-        DMRG_CUDA(launch_shape(*l.ph, l.shape, ex->w[i % nw]));
-      }
-      for (int i = 0; i < nw; ++i) {
-        DMRG_CUDA(cudaEventRecord(ex->join[i], ex->w[i]));
-        DMRG_CUDA(cudaStreamWaitEvent(st, ex->join[i], 0));
-      }
+      if (launch_counter) *launch_counter += (int64_t)ls.size();
+      for (int i = 0; i < LA; ++i)
+        DMRG_CUDA(cudaStreamWaitEvent(ex->w[i], c < 2 ? ex->fork : evDone(c - 2), 0));
+      for (size_t q = 0; q < ls.size(); ++q) DMRG_CUDA(launch_shape(*ls[q].ph, ls[q].shape, ex->w[q % LA]));
+      for (int i = 0; i < LA; ++i) DMRG_CUDA(cudaEventRecord(evA(c, i), ex->w[i]));
     }
-    if (stage > 0 && chunks[stage - 1].p2.nred > 0) {
-      const Phase& ph = chunks[stage - 1].p2;
-      launch_reduce_partials(ph.red.p, ph.nred, ph.red_max_batch, st);
-      if (launch_counter) ++*launch_counter;
+    // ---- lane B: phase 2 of chunk c, then its split-K reduction ----
+    {
+      const Phase& ph = chunks[c].p2;
+      std::vector<Launch> ls;
+      collect(ph, ls);
+      std::stable_sort(ls.begin(), ls.end(), [](const Launch& a, const Launch& b) { return a.work > b.work; });
+      if (launch_counter) *launch_counter += (int64_t)ls.size() + (ph.nred > 0);
+      for (int j = 0; j < LB; ++j) {
+        for (int i = 0; i < LA; ++i) DMRG_CUDA(cudaStreamWaitEvent(ex->w[LA + j], evA(c, i), 0));
+        if (c > 0) DMRG_CUDA(cudaStreamWaitEvent(ex->w[LA + j], evDone(c - 1), 0));
+      }
+      for (size_t q = 0; q < ls.size(); ++q) DMRG_CUDA(launch_shape(*ls[q].ph, ls[q].shape, ex->w[LA + q % LB]));
+      for (int j = 1; j < LB; ++j) {
+        DMRG_CUDA(cudaEventRecord(evB(c, j), ex->w[LA + j]));
+        DMRG_CUDA(cudaStreamWaitEvent(ex->w[LA], evB(c, j), 0));
+      }
+      if (ph.nred > 0) launch_reduce_partials(ph.red.p, ph.nred, ph.red_max_batch, ex->w[LA]);
+      DMRG_CUDA(cudaEventRecord(evDone(c), ex->w[LA]));
     }
   }
+  DMRG_CUDA(cudaStreamWaitEvent(st, evDone(n - 1), 0));
+  for (int i = 0; i < LA; ++i) DMRG_CUDA(cudaStreamWaitEvent(st, evA(n - 1, i), 0));
 }
 
 void Plan::run_profiled(cudaStream_t st, std::vector<LaunchRecord>* out) const {

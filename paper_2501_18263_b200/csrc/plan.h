@@ -88,6 +88,8 @@ struct Exec {
   static constexpr int NW = 6;
   cudaStream_t w[NW] = {};
   cudaEvent_t fork = nullptr, join[NW] = {};
+  std::vector<cudaEvent_t> pool;      // per-chunk events of Plan::run's two lanes (created on first use, kept)
+  cudaEvent_t event(size_t i);
   bool ok = false;
   void init();
   ~Exec();
@@ -106,9 +108,11 @@ struct Plan {
   double flops_shared = 0;   // phase-1 flops saved by sharing intermediates between term groups
   int64_t n_items = 0, n_products = 0;
   int launches() const;
-  // Stages: P1(0) | P2(c-1) + P1(c) ... | P2(last); the launches of a stage are independent (phase 1 of
-  // chunk c writes workspace half c&1 while phase 2 of chunk c-1 reads the other half) and run on the
-  // worker streams of `ex` (nullptr: everything in order on `st`).
+  // Two lanes on the worker streams of `ex` (nullptr: everything in order on `st`): lane A runs phase 1 of the
+  // chunks, lane B phase 2 and the split-K reductions.  Dependencies are per chunk, by events: phase 1 of chunk c
+  // needs workspace half c&1 back (phase 2 of chunk c-2 done), phase 2 of chunk c needs phase 1 of chunk c and
+  // phase 2 of chunk c-1 (outputs accumulate in chunk order: no atomics, fixed order).  No stage-wide joins:
+  // the tail of one launch is filled by whatever the other lane has ready.
   void run(cudaStream_t st, int64_t* launch_counter, Exec* ex = nullptr) const;
   // Same launches, each bracketed by events (shape -1 = split-K reduction).  Synchronises `st`.
   void run_profiled(cudaStream_t st, std::vector<LaunchRecord>* out) const;
