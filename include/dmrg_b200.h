@@ -177,6 +177,30 @@ int dmrg_heff_apply_host(dmrg_ctx* ctx, const double* h_psi_in, double* h_psi_ou
 int dmrg_davidson_host(dmrg_ctx* ctx, double* h_psi, double tol, int32_t max_iter, int32_t max_basis,
                        double* h_energy, int32_t* h_iters, double* h_resid, void* stream);
 
+/* ---- mode-optimisation micro-iteration (Sec. II.B, :57-75, Fig. 1 :63), steps ii) and iii); U(1)xU(1) ----
+ *
+ * dmrg_two_site_gate: psi_out{a, s1' s2', b} = sum_{s1 s2} G[(s1' s2'), (s1 s2)] psi_in{a, s1 s2, b} for a 16 x 16
+ * row-major gate h_G on the occupation basis of sites k, k+1 (index 4 s1 + s2).  G must conserve (n_up, n_dn) of the
+ * pair (DMRG_ERR_INPUT otherwise).  For the orbital rotation c~+_k = cos(theta) c+_k + sin(theta) c+_{k+1},
+ * c~+_{k+1} = -sin(theta) c+_k + cos(theta) c+_{k+1} (both spins), the coefficients of the same state in the rotated
+ * modes are G = exp(-theta kappa) psi with kappa = sum_s (c+_{k+1,s} c_{k,s} - c+_{k,s} c_{k+1,s}); theta = pi/2 is the
+ * swap gate of PAPER.md:89 up to signs.  d_psi_in and d_psi_out must not alias.  Synchronises `stream`.
+ *
+ * dmrg_bond_entropy: block entropies of rho_{1..k} (the cut between the two sites) of the two-site wavefunction
+ * d_psi: *h_S_half = S_1/2 = 2 ln Tr sqrt(rho) (the cost function of PAPER.md:75), *h_S_vn = -Tr rho ln rho; psi is
+ * normalised internally.  The singular values of Psi[(a s_k), (s_{k+1} b)] are computed per sector of bond k by a
+ * one-sided Jacobi kernel in shared memory (DMRG_ERR_UNSUPPORTED if a sector exceeds ~160 x 160: the paper runs mode
+ * optimisation at D <= 256); h_sigma (optional, host) receives them unnormalised, sector by sector
+ * (sectors of bond k in lexicographic order), *n_sigma their number.  Any output pointer may be NULL.
+ *
+ * dmrg_rotate_integrals: T and V are replaced by the integrals in the rotated modes (k, k+1 1-based sites,
+ * same theta convention), so that H is unchanged as an operator; all environments become invalid
+ * (call dmrg_env_build again).  Host work only. */
+int dmrg_two_site_gate(dmrg_ctx* ctx, const double* h_G, const double* d_psi_in, double* d_psi_out, void* stream);
+int dmrg_bond_entropy(dmrg_ctx* ctx, const double* d_psi, double* h_S_half, double* h_S_vn, double* h_sigma,
+                      int32_t* n_sigma, void* stream);
+int dmrg_rotate_integrals(dmrg_ctx* ctx, int32_t k, double theta);
+
 typedef struct {
   int64_t n_terms;          /* four-part terms of PAPER.md Eq. (6) after pre-summation */
   int64_t n_tasks;          /* (term x sector) tasks of PAPER.md Eq. (8) */

@@ -23,6 +23,7 @@ EXPORTS = [
     "dmrg_heff_diag", "dmrg_davidson", "dmrg_heff_apply_host", "dmrg_davidson_host", "dmrg_stats",
     "dmrg_env_export", "dmrg_fp64_peak", "dmrg_apply_profile", "dmrg_mps_set_site_su2", "dmrg_su2_f_factor",
     "dmrg_mps_update_bond", "dmrg_set_shard", "dmrg_shard_info", "dmrg_env_export_block", "dmrg_block_flops", "dmrg_dfma_peak",
+    "dmrg_two_site_gate", "dmrg_bond_entropy", "dmrg_rotate_integrals",
 ]
 
 REDUCE_FN = C.CFUNCTYPE(C.c_int, C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p)
@@ -100,6 +101,9 @@ def load_library(build_if_missing: bool = True):
     lib.dmrg_fp64_peak.argtypes = [vp, dp, vp]
     lib.dmrg_dfma_peak.argtypes = [vp, dp, vp]
     lib.dmrg_block_flops.argtypes = [vp, vp]
+    lib.dmrg_two_site_gate.argtypes = [vp, vp, vp, vp, vp]
+    lib.dmrg_bond_entropy.argtypes = [vp, vp, dp, dp, vp, C.POINTER(i32), vp]
+    lib.dmrg_rotate_integrals.argtypes = [vp, i32, C.c_double]
     lib.dmrg_apply_profile.argtypes = [vp, vp, vp, i32, C.POINTER(LaunchInfo), C.POINTER(i32), vp]
     for name in EXPORTS:
         if name != "dmrg_last_error":
@@ -350,6 +354,31 @@ class DMRG:
         out = np.zeros(len(self.psi_layout()[0]))
         self._check(self.lib.dmrg_block_flops(self.ctx, _np_ptr(out)))
         return out
+
+    def two_site_gate(self, G, psi_in, psi_out=None):
+        """psi_out = (16 x 16 gate on the occupation basis of sites k, k+1) applied to psi_in (CUDA tensors)."""
+        G = np.ascontiguousarray(G, dtype=np.float64)
+        assert G.shape == (16, 16)
+        if psi_out is None:
+            psi_out = self.torch.empty_like(psi_in)
+        self._check(self.lib.dmrg_two_site_gate(self.ctx, _np_ptr(G), C.c_void_p(psi_in.data_ptr()),
+                                                C.c_void_p(psi_out.data_ptr()), self._stream()))
+        return psi_out
+
+    def bond_entropy(self, psi, spectrum=False):
+        """(S_1/2, S_1[, singular values]) of the cut between sites k and k+1 of the two-site wavefunction psi."""
+        a, b, n = C.c_double(), C.c_double(), C.c_int32()
+        self._check(self.lib.dmrg_bond_entropy(self.ctx, C.c_void_p(psi.data_ptr()), C.byref(a), C.byref(b), None,
+                                               C.byref(n), self._stream()))
+        if not spectrum:
+            return a.value, b.value
+        sig = np.zeros(max(n.value, 1))
+        self._check(self.lib.dmrg_bond_entropy(self.ctx, C.c_void_p(psi.data_ptr()), C.byref(a), C.byref(b), _np_ptr(sig),
+                                               C.byref(n), self._stream()))
+        return a.value, b.value, sig[:n.value]
+
+    def rotate_integrals(self, k, theta):
+        self._check(self.lib.dmrg_rotate_integrals(self.ctx, int(k), float(theta)))
 
     def apply_profile(self, psi_in, psi_out=None, cap=4096):
         """One H_eff.psi with per-launch event timing; returns (psi_out, list of dict per launch)."""
