@@ -197,6 +197,8 @@ int dmrg_davidson_host(dmrg_ctx* ctx, double* h_psi, double tol, int32_t max_ite
  * same theta convention), so that H is unchanged as an operator; all environments become invalid
  * (call dmrg_env_build again).  Host work only. */
 int dmrg_two_site_gate(dmrg_ctx* ctx, const double* h_G, const double* d_psi_in, double* d_psi_out, void* stream);
+/* h_G (16 x 16, row-major) = exp(-theta kappa), the gate of the orbital rotation described above (host). */
+int dmrg_rotation_gate(double theta, double* h_G);
 int dmrg_bond_entropy(dmrg_ctx* ctx, const double* d_psi, double* h_S_half, double* h_S_vn, double* h_sigma,
                       int32_t* n_sigma, void* stream);
 int dmrg_rotate_integrals(dmrg_ctx* ctx, int32_t k, double theta);

@@ -23,7 +23,7 @@ EXPORTS = [
     "dmrg_heff_diag", "dmrg_davidson", "dmrg_heff_apply_host", "dmrg_davidson_host", "dmrg_stats",
     "dmrg_env_export", "dmrg_fp64_peak", "dmrg_apply_profile", "dmrg_mps_set_site_su2", "dmrg_su2_f_factor",
     "dmrg_mps_update_bond", "dmrg_set_shard", "dmrg_shard_info", "dmrg_env_export_block", "dmrg_block_flops", "dmrg_dfma_peak",
-    "dmrg_two_site_gate", "dmrg_bond_entropy", "dmrg_rotate_integrals",
+    "dmrg_two_site_gate", "dmrg_bond_entropy", "dmrg_rotate_integrals", "dmrg_rotation_gate",
 ]
 
 REDUCE_FN = C.CFUNCTYPE(C.c_int, C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p)
@@ -104,6 +104,7 @@ def load_library(build_if_missing: bool = True):
     lib.dmrg_two_site_gate.argtypes = [vp, vp, vp, vp, vp]
     lib.dmrg_bond_entropy.argtypes = [vp, vp, dp, dp, vp, C.POINTER(i32), vp]
     lib.dmrg_rotate_integrals.argtypes = [vp, i32, C.c_double]
+    lib.dmrg_rotation_gate.argtypes = [C.c_double, vp]
     lib.dmrg_apply_profile.argtypes = [vp, vp, vp, i32, C.POINTER(LaunchInfo), C.POINTER(i32), vp]
     for name in EXPORTS:
         if name != "dmrg_last_error":
@@ -399,6 +400,16 @@ class DMRG:
         for i, blocks in mps.right.items():
             put(i, 1, blocks)
         self.env_build(mps.k)
+
+
+def rotation_gate(theta):
+    """16 x 16 gate exp(-theta kappa) of the two-site orbital rotation (dmrg_rotation_gate)."""
+    lib = load_library()
+    G = np.zeros((16, 16))
+    rc = lib.dmrg_rotation_gate(float(theta), _np_ptr(G))
+    if rc != 0:
+        raise DMRGError("dmrg_rotation_gate failed with status %d" % rc)
+    return G
 
 
 def su2_f_factor(Sa, Sk, Sg, kL, kk, k, Sa_, Sk_, Sg_):

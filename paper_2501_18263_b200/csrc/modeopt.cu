@@ -189,6 +189,57 @@ int dmrg_two_site_gate(dmrg_ctx* ctx, const double* h_G, const double* d_in, dou
   MO_END
 }
 
+int dmrg_rotation_gate(double theta, double* h_G) {
+  if (!h_G) return DMRG_ERR_ARG;
+  // kappa = sum_s (c+_{2,s} c_{1,s} - c+_{1,s} c_{2,s}) on the two-site occupation basis (index 4 s1 + s2), Jordan-Wigner:
+  // c+_{1,s} = c+_s (x) 1, c+_{2,s} = P (x) c+_s with the site matrices of DESIGN.md "Conventions"
+  double cre[2][16] = {}, par[16] = {}, one[16] = {};
+  cre[0][2 * 4 + 0] = 1.0; cre[0][3 * 4 + 1] = 1.0;       // a+_up : 0 -> up, dn -> up+dn
+  cre[1][1 * 4 + 0] = 1.0; cre[1][3 * 4 + 2] = -1.0;      // a+_dn : 0 -> dn, up -> -(up+dn)
+  const double pd[4] = {1.0, -1.0, -1.0, 1.0};
+  for (int i = 0; i < 4; ++i) { par[i * 4 + i] = pd[i]; one[i * 4 + i] = 1.0; }
+  auto kron = [](const double* a, const double* b, double* o) {
+    for (int r1 = 0; r1 < 4; ++r1) for (int c1 = 0; c1 < 4; ++c1) for (int r2 = 0; r2 < 4; ++r2) for (int c2 = 0; c2 < 4; ++c2)
+      o[(r1 * 4 + r2) * 16 + c1 * 4 + c2] = a[r1 * 4 + c1] * b[r2 * 4 + c2];
+  };
+  double K[256] = {};
+  for (int s = 0; s < 2; ++s) {
+    double c1[256], c2[256];
+    kron(cre[s], one, c1);
+    kron(par, cre[s], c2);
+    for (int r = 0; r < 16; ++r) for (int c = 0; c < 16; ++c) {
+      double v = 0.0;
+      for (int q = 0; q < 16; ++q) v += c2[r * 16 + q] * c1[c * 16 + q] - c1[r * 16 + q] * c2[c * 16 + q];   // c2 c1^T - c1 c2^T
+      K[r * 16 + c] += v;
+    }
+  }
+  // G = exp(-theta K): scaling and squaring of the Taylor series
+  int sq = 0;
+  double t = -theta;
+  while (std::fabs(t) > 0.125) { t *= 0.5; ++sq; }
+  double G[256] = {}, term[256] = {}, tmp[256];
+  for (int i = 0; i < 16; ++i) G[i * 16 + i] = term[i * 16 + i] = 1.0;
+  for (int n = 1; n <= 24; ++n) {
+    for (int r = 0; r < 16; ++r) for (int c = 0; c < 16; ++c) {
+      double v = 0.0;
+      for (int q = 0; q < 16; ++q) v += term[r * 16 + q] * K[q * 16 + c];
+      tmp[r * 16 + c] = v * t / n;
+    }
+    std::memcpy(term, tmp, sizeof(tmp));
+    for (int i = 0; i < 256; ++i) G[i] += term[i];
+  }
+  for (int s = 0; s < sq; ++s) {
+    for (int r = 0; r < 16; ++r) for (int c = 0; c < 16; ++c) {
+      double v = 0.0;
+      for (int q = 0; q < 16; ++q) v += G[r * 16 + q] * G[q * 16 + c];
+      tmp[r * 16 + c] = v;
+    }
+    std::memcpy(G, tmp, sizeof(tmp));
+  }
+  std::memcpy(h_G, G, sizeof(G));
+  return DMRG_OK;
+}
+
 int dmrg_bond_entropy(dmrg_ctx* ctx, const double* d_psi, double* h_S_half, double* h_S_vn, double* h_sigma,
                       int32_t* n_sigma, void* stream) {
   MO_BEGIN
