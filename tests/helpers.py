@@ -77,3 +77,17 @@ def embedding(mps, psi_blocks):
         P[rows[~bad], off:off + dL * dR] += blockP[~bad]
         off += dL * dR
     return P, dets
+
+
+def assert_blocks_close(got, ref, sizes, rel=1e-11):
+    """Whole-vector rel-L2 <= rel (the north_star tolerance) AND, block by block, max |got - ref| small against the
+    block's own scale: an error confined to one small psi block does not show in the whole-vector norm."""
+    got, ref = np.asarray(got), np.asarray(ref)
+    assert np.linalg.norm(got - ref) / np.linalg.norm(ref) <= rel
+    floor = 1e-3 * np.abs(ref).max()
+    o = 0
+    for n in sizes:
+        g, r = got[o:o + n], ref[o:o + n]
+        assert np.abs(g - r).max() <= 10 * rel * (np.abs(r).max() + floor), (o, n)
+        o += n
+    assert o == len(ref)

@@ -7,6 +7,7 @@ Tolerances (BASELINE.json north_star; R18): rel-L2 <= 1e-11 on H_eff.p
 import numpy as np
 import pytest
 
+from helpers import assert_blocks_close
 from oracle import dmrg as odmrg
 from oracle import fci
 from paper_2501_18263_b200 import inputs
@@ -55,7 +56,11 @@ def _general_integrals(L, seed):
     (6, 4, 0, 3, 10 ** 9),                                                  # no down electrons at all
     (8, 4, 4, 4, 40),                                                       # several ragged sectors per tile
 ])
-def test_apply_and_diag_small(L, nu, nd, k, D):
+@pytest.mark.parametrize("path", ["fused", "two_phase"])
+def test_apply_and_diag_small(L, nu, nd, k, D, path, monkeypatch):
+    # at these sizes every task fits the fused small-sector kernel; the second run forces the two-phase grouped GEMM
+    if path == "two_phase":
+        monkeypatch.setenv("DMRG_B200_NO_FUSED", "1")
     T, V = _general_integrals(L, 100 + L + k)
     mps = inputs.make_mps(L, nu, nd, D, k, seed=5)
     orc = _oracle(T, V, mps)
@@ -69,8 +74,58 @@ def test_apply_and_diag_small(L, nu, nd, k, D):
     rng = np.random.default_rng(1)
     for _ in range(2):
         v = rng.normal(size=n)
-        assert _rel(_apply_gpu(d, v), orc.apply(v)) <= REL_L2
+        assert_blocks_close(_apply_gpu(d, v), orc.apply(v), [b[4] * b[5] for b in ref_blocks], REL_L2)
     assert np.abs(d.heff_diag().cpu().numpy() - orc.diag()).max() <= 1e-11
+    d.close()
+
+
+def test_davidson_with_a_core_energy():
+    """e_core shifts H_eff by a constant: the same iterates, E = E(e_core = 0) + e_core, and the residual criterion is met
+    (the residual is formed with the Ritz value of the shifted operator, the preconditioner with the unshifted diagonal)."""
+    import torch
+    from paper_2501_18263_b200.binding import DMRG
+    T, V = inputs.make_integrals(8, 31)
+    mps = inputs.make_mps(8, 4, 4, 40, 4, seed=6)
+    v0 = inputs.make_psi0(mps, 3)
+    res = []
+    for e_core in (0.0, -37.25):
+        d = DMRG(8, 4, 4)
+        d.setup(T, V, mps, e_core=e_core)
+        x = torch.from_numpy(v0.copy()).cuda()
+        E, it, rn = d.davidson(x, tol=1e-9, max_iter=300, max_basis=16)
+        assert rn <= 1e-9 and it < 300
+        res.append((E, it, x.cpu().numpy()))
+        d.close()
+    assert abs(res[1][0] - (res[0][0] - 37.25)) <= 1e-9
+    assert abs(res[0][1] - res[1][1]) <= 8        # same algorithm; the shift changes the rounding, not the convergence
+    assert abs(abs(res[0][2] @ res[1][2]) - 1.0) <= 1e-8
+
+
+def test_small_workspace_splits_and_chunks(monkeypatch):
+    """workspace_bytes far below one chunk: apply and renormalisation run in many chunks with split batched items
+    (Planner::add); results unchanged against the oracle.  (Two-phase path forced: the fused kernel has no workspace.)"""
+    monkeypatch.setenv("DMRG_B200_NO_FUSED", "1")
+    L, nu, nd, k, D = 8, 4, 4, 3, 40
+    T, V = _general_integrals(L, 77)
+    sectors = inputs.bond_sectors(L, nu, nd, D)
+    a = inputs.make_mps(L, nu, nd, D, k, seed=5, sectors=sectors)
+    b = inputs.make_mps(L, nu, nd, D, k + 1, seed=6, sectors=sectors)
+    start = inputs.MPSInput(L=L, k=k, n_up=nu, n_dn=nd, sectors=sectors,
+                            left={i: b.left[i] for i in range(1, k)}, right=a.right)
+    ref_blocks = inputs.psi_blocks(start)
+    orc = _oracle(T, V, start)
+    d = _gpu(T, V, start, workspace_bytes=48 << 10)
+    assert d.stats()["n_chunks"] >= 4
+    v = np.random.default_rng(2).normal(size=d.psi_size())
+    assert_blocks_close(_apply_gpu(d, v), orc.apply(v), [q[4] * q[5] for q in ref_blocks], REL_L2)
+    d.mps_set_site(k, 0, b.left[k])
+    d.renormalize(0)
+    m2 = inputs.MPSInput(L=L, k=k + 1, n_up=nu, n_dn=nd, sectors=sectors, left=b.left,
+                         right={i: a.right[i] for i in range(k + 3, L + 1)})
+    orc2 = _oracle(T, V, m2)
+    v2 = np.random.default_rng(3).normal(size=d.psi_size())
+    assert d.psi_size() == orc2.psi_size()
+    assert_blocks_close(_apply_gpu(d, v2), orc2.apply(v2), [q[4] * q[5] for q in inputs.psi_blocks(m2)], REL_L2)
     d.close()
 
 

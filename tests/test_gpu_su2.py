@@ -5,6 +5,7 @@ Tolerances as for U(1): rel-L2 <= 1e-11 on H_eff.psi, |dE| <= 1e-9 Eh on Davidso
 import numpy as np
 import pytest
 
+from helpers import assert_blocks_close
 from oracle import dmrg as odmrg
 from oracle import fci, su2
 from paper_2501_18263_b200 import inputs
@@ -64,7 +65,7 @@ def test_su2_apply_and_layout(L, N, k, D):
     rng = np.random.default_rng(1)
     for _ in range(2):
         v = rng.normal(size=n)
-        assert _rel(_apply_gpu(d, v), orc.apply(v)) <= REL_L2
+        assert_blocks_close(_apply_gpu(d, v), orc.apply(v), [q[5] * q[6] for q in ref_blocks], REL_L2)
     d.close()
 
 
