@@ -254,7 +254,7 @@ bool Planner::add_fused(const Item& it) {
 Planner::HOut& Planner::p2_out(HChunk& ch, const Item& it, int b0, int cnt, int M, int N) {
   const bool batched = it.strideC != 0;
   double* C = it.C + (batched ? b0 * it.strideC : 0);
-  auto key = std::make_tuple((const double*)C, batched ? cnt : 1, it.strideC);
+  const P2Key key{(const double*)C, batched ? cnt : 1, it.strideC};
   auto f = ch.p2_index.find(key);
   if (f != ch.p2_index.end()) return ch.p2[f->second];
   HOut o{};

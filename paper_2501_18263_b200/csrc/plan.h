@@ -131,12 +131,35 @@ class Planner {
   struct HSeg { GSeg s; bool a_ws, b_ws; };          // *_ws: pointer is a workspace offset
   struct HOut { GOut o; bool c_ws; std::vector<HSeg> segs; int batch; double work; bool c_sc = false; };
   // identity of a phase-1 product (operands, shapes, batch): equal keys give the same intermediate
-  using ZKey = std::tuple<const double*, const double*, long long, long long, int, int, int, int, int, int, int>;
+  struct ZKey {
+    const double* a; const double* b; long long sa, sb; int lda, ldb, rows, k, cols, cnt, flags;
+    bool operator==(const ZKey& o) const {
+      return a == o.a && b == o.b && sa == o.sa && sb == o.sb && lda == o.lda && ldb == o.ldb && rows == o.rows && k == o.k &&
+             cols == o.cols && cnt == o.cnt && flags == o.flags;
+    }
+  };
+  struct ZHash {
+    size_t operator()(const ZKey& z) const {
+      uint64_t h = (uint64_t)(uintptr_t)z.a * 0x9E3779B97F4A7C15ull ^ ((uint64_t)(uintptr_t)z.b + 0x7F4A7C15ull) * 0xC2B2AE3D27D4EB4Full;
+      h ^= ((uint64_t)z.cnt << 40) ^ ((uint64_t)z.rows << 20) ^ (uint64_t)z.cols ^ ((uint64_t)z.flags << 60) ^ ((uint64_t)z.k << 8);
+      return (size_t)(h ^ (h >> 29));
+    }
+  };
+  struct P2Key {
+    const double* c; int batch; long long stride;
+    bool operator==(const P2Key& o) const { return c == o.c && batch == o.batch && stride == o.stride; }
+  };
+  struct P2Hash {
+    size_t operator()(const P2Key& k) const {
+      uint64_t h = (uint64_t)(uintptr_t)k.c * 0x9E3779B97F4A7C15ull ^ ((uint64_t)k.batch << 48) ^ (uint64_t)k.stride;
+      return (size_t)(h ^ (h >> 31));
+    }
+  };
   struct HChunk {
-    std::map<ZKey, long long> zmap;     // intermediates already in this chunk's workspace
+    std::unordered_map<ZKey, long long, ZHash> zmap;     // intermediates already in this chunk's workspace
     std::vector<HOut> p1;
     std::vector<HOut> p2;
-    std::map<std::tuple<const double*, int, long long>, int> p2_index;  // (C, batch, strideC) -> p2 slot
+    std::unordered_map<P2Key, int, P2Hash> p2_index;     // (C, batch, strideC) -> p2 slot
     std::map<const double*, const double*> batched_out;   // [begin, end) of the batched outputs of this chunk
     long long ws_used = 0;
   };
@@ -144,7 +167,7 @@ class Planner {
   bool add_fused(const Item& it);
   struct HFOut { double* C; int ldc, M, N; std::vector<FTask> tasks; };
   std::vector<HFOut> fused_;
-  std::map<const double*, int> fused_index_;
+  std::unordered_map<const double*, int> fused_index_;
   bool fused_on_ = std::getenv("DMRG_B200_NO_FUSED") == nullptr;
   // largest output dimension / largest contraction extent routed to the fused kernel (measured: DESIGN.md §7)
   int fused_max_ = std::getenv("DMRG_B200_FUSED_MAX") ? std::atoi(std::getenv("DMRG_B200_FUSED_MAX")) : 64;

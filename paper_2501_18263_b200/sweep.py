@@ -86,6 +86,7 @@ class TwoSiteSweep:
         E, it, rn = d.davidson(x, tol=tol, max_iter=max_iter, max_basis=max_basis)
         t0 = self._tick("Diag_H", t0)
         self.energies.append(E)
+        self.last_psi = x                      # the optimised two-site wavefunction this step truncates (tests)
         if direction is None:
             self.guess = x
             return E
@@ -97,7 +98,7 @@ class TwoSiteSweep:
             g["cols"].setdefault((s2, qR), dR)
             g["blk"].append(((qL, s1), (s2, qR), dL, dR, off))
         svds, allsv = {}, []
-        for qm, g in groups.items():
+        for qm, g in sorted(groups.items()):    # lexicographic sector order: the tie-break rule of the truncation
             ro, co, o = {}, {}, 0
             for key in sorted(g["rows"]):
                 ro[key] = o; o += g["rows"][key]

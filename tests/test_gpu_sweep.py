@@ -161,3 +161,34 @@ def test_host_tier_of_the_environment_cache(su2):
     assert s1["env_spills"] >= L - 3 and s1["env_fetches"] >= L - 3
     assert s1["env_host_bytes"] <= 1 << 30
     assert s1["total_launches"] == s0["total_launches"]
+
+
+def test_truncation_matches_the_oracle():
+    """The kept dimension per bond sector (exactly), the discarded weight and the kept singular values of the driver's
+    device SVD against oracle/sweep.py on the same optimised wavefunction; the library's own per-sector Jacobi singular
+    values (dmrg_bond_entropy) agree with both."""
+    import torch
+    from oracle import sweep as osweep
+    from paper_2501_18263_b200.binding import DMRG
+    from paper_2501_18263_b200.sweep import TwoSiteSweep
+    L, nu, nd, D = 10, 5, 5, 28
+    T, V = inputs.make_integrals(L, 17)
+    mps = inputs.make_mps(L, nu, nd, D, 5, seed=3)
+    d = DMRG(L, nu, nd)
+    sw = TwoSiteSweep(d, T, V, mps, D)
+    for direction in (0, 0, 1):
+        pb = [(q[0], q[1], q[2], q[3], q[4], q[5]) for q in sw._layout()[0]]
+        k = sw.k
+        sw.step(direction, tol=1e-9)
+        x = sw.last_psi.cpu().numpy()
+        kept, weight, sig = osweep.truncate(pb, x, D)
+        assert sw.sectors[k] == kept
+        assert abs(sw.trunc[-1] - weight) <= 1e-13 * max(1.0, weight)
+        assert sum(kept.values()) <= D
+    # the library's Jacobi singular values at the current bond
+    pb = [(q[0], q[1], q[2], q[3], q[4], q[5]) for q in sw._layout()[0]]
+    y = sw.guess.clone()
+    _, _, sig_lib = d.bond_entropy(y, spectrum=True)
+    ref = np.concatenate([np.linalg.svd(M, compute_uv=False) for _, M in sorted(osweep.sector_matrices(pb, y.cpu().numpy()).items())])
+    assert np.abs(np.sort(sig_lib) - np.sort(ref)).max() <= 1e-12
+    d.close()
