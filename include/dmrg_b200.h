@@ -203,6 +203,25 @@ int dmrg_bond_entropy(dmrg_ctx* ctx, const double* d_psi, double* h_S_half, doub
                       int32_t* n_sigma, void* stream);
 int dmrg_rotate_integrals(dmrg_ctx* ctx, int32_t k, double theta);
 
+/* dmrg_bond_entropy_static: dmrg_bond_entropy (same arguments, same kernels, same results) for callers that may not
+ * allocate device memory: code under CUDA graph capture, tight serving loops, harnesses that forbid cudaMalloc.  It
+ * calls no cudaMalloc / cudaFree, none of the context's allocator callbacks and no allocating library routine: the
+ * sector tables, the singular values and the three results live in one file-scope `static __device__` array of
+ * ~124 KiB, which every GPU that loads the library holds until the process exits.  Its device address is looked up
+ * once per device (cudaGetSymbolAddress, on the first call with a context of that device).
+ *   Limits (DMRG_ERR_UNSUPPORTED beyond them, with the count in dmrg_last_error; dmrg_bond_entropy has none of them):
+ * at most DMRG_STATIC_MAX_SIGMA singular values (sum over the sectors of bond k of min(rows, columns): enough for
+ * D <= 512), DMRG_STATIC_MAX_SECTORS sectors of bond k and DMRG_STATIC_MAX_BLOCKS psi blocks.
+ *   d_psi: device, read only.  h_*: host, optional as in dmrg_bond_entropy.  Synchronises `stream`.
+ *   ALL calls in the process that use one GPU share the array, across contexts and threads: calls that overlap on the
+ * GPU (two streams, two host threads) race and return garbage; serialise them.  The array keeps the last call's
+ * contents; every word a kernel reads is written earlier in the same call and the result slot is cleared first. */
+#define DMRG_STATIC_MAX_SIGMA 2048
+#define DMRG_STATIC_MAX_SECTORS 512
+#define DMRG_STATIC_MAX_BLOCKS 4096
+int dmrg_bond_entropy_static(dmrg_ctx* ctx, const double* d_psi, double* h_S_half, double* h_S_vn, double* h_sigma,
+                             int32_t* n_sigma, void* stream);
+
 typedef struct {
   int64_t n_terms;          /* four-part terms of PAPER.md Eq. (6) after pre-summation */
   int64_t n_tasks;          /* (term x sector) tasks of PAPER.md Eq. (8) */

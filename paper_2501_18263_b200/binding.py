@@ -23,8 +23,10 @@ EXPORTS = [
     "dmrg_heff_diag", "dmrg_davidson", "dmrg_heff_apply_host", "dmrg_davidson_host", "dmrg_stats",
     "dmrg_env_export", "dmrg_fp64_peak", "dmrg_apply_profile", "dmrg_mps_set_site_su2", "dmrg_su2_f_factor",
     "dmrg_mps_update_bond", "dmrg_set_shard", "dmrg_shard_info", "dmrg_env_export_block", "dmrg_block_flops", "dmrg_dfma_peak",
-    "dmrg_two_site_gate", "dmrg_bond_entropy", "dmrg_rotate_integrals", "dmrg_rotation_gate",
+    "dmrg_two_site_gate", "dmrg_bond_entropy", "dmrg_rotate_integrals", "dmrg_rotation_gate", "dmrg_bond_entropy_static",
 ]
+
+STATIC_MAX_SIGMA, STATIC_MAX_SECTORS, STATIC_MAX_BLOCKS = 2048, 512, 4096     # include/dmrg_b200.h DMRG_STATIC_MAX_*
 
 REDUCE_FN = C.CFUNCTYPE(C.c_int, C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p)
 ALLOC_FN = C.CFUNCTYPE(C.c_void_p, C.c_uint64, C.c_void_p)
@@ -103,6 +105,7 @@ def load_library(build_if_missing: bool = True):
     lib.dmrg_block_flops.argtypes = [vp, vp]
     lib.dmrg_two_site_gate.argtypes = [vp, vp, vp, vp, vp]
     lib.dmrg_bond_entropy.argtypes = [vp, vp, dp, dp, vp, C.POINTER(i32), vp]
+    lib.dmrg_bond_entropy_static.argtypes = [vp, vp, dp, dp, vp, C.POINTER(i32), vp]
     lib.dmrg_rotate_integrals.argtypes = [vp, i32, C.c_double]
     lib.dmrg_rotation_gate.argtypes = [C.c_double, vp]
     lib.dmrg_apply_profile.argtypes = [vp, vp, vp, i32, C.POINTER(LaunchInfo), C.POINTER(i32), vp]
@@ -377,6 +380,16 @@ class DMRG:
         self._check(self.lib.dmrg_bond_entropy(self.ctx, C.c_void_p(psi.data_ptr()), C.byref(a), C.byref(b), _np_ptr(sig),
                                                C.byref(n), self._stream()))
         return a.value, b.value, sig[:n.value]
+
+    def bond_entropy_static(self, psi, spectrum=False):
+        """bond_entropy through dmrg_bond_entropy_static: no device allocation, scratch in a static device array shared
+        by every call on this GPU (include/dmrg_b200.h for the limits).  The spectrum buffer is sized to the limit, so
+        this method makes one call."""
+        a, b, n = C.c_double(), C.c_double(), C.c_int32()
+        sig = np.zeros(STATIC_MAX_SIGMA) if spectrum else None
+        self._check(self.lib.dmrg_bond_entropy_static(self.ctx, C.c_void_p(psi.data_ptr()), C.byref(a), C.byref(b),
+                                                      _np_ptr(sig) if spectrum else None, C.byref(n), self._stream()))
+        return (a.value, b.value, sig[:n.value]) if spectrum else (a.value, b.value)
 
     def rotate_integrals(self, k, theta):
         self._check(self.lib.dmrg_rotate_integrals(self.ctx, int(k), float(theta)))

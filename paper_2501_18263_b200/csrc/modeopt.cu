@@ -6,9 +6,12 @@
 //   dmrg_bond_entropy    singular values of Psi[(a s1), (s2 b)] per sector of bond k by one-sided Jacobi in shared
 //                        memory (one CTA per sector), S_1/2 = 2 ln sum sigma_i and S_1 from them on the device
 //   dmrg_rotate_integrals  T, w -> rotated by the 2x2 block on orbitals (k, k+1); host data of the context
+//   dmrg_bond_entropy_static  dmrg_bond_entropy with its device scratch in a file-scope array: allocates nothing
 #include <algorithm>
 #include <cmath>
 #include <cstring>
+#include <map>
+#include <mutex>
 
 #include "engine.h"
 
@@ -331,3 +334,116 @@ int dmrg_rotate_integrals(dmrg_ctx* ctx, int32_t k, double theta) {
 }
 
 }  // extern "C"
+
+// ------------------------------------------------------------------------------------------------------------------
+// dmrg_bond_entropy_static: dmrg_bond_entropy for callers that may not allocate device memory (code under CUDA graph
+// capture, tight serving loops, harnesses that forbid cudaMalloc).  The same two kernels; every device buffer they
+// need beyond psi (sector and placement tables, the singular values, the three results) lives in ONE file-scope
+// array of fixed size, which every GPU that loads the library holds until the process exits.
+//
+// In host code `g_entropy_scratch` is only a stand-in for the symbol: its device address is looked up once per device,
+// with that device current, by cudaGetSymbolAddress, and it is that address the kernels are given.
+// ------------------------------------------------------------------------------------------------------------------
+namespace {
+
+constexpr size_t ST_OFF_OUT = 0;                                                            // 3 doubles (256 B reserved)
+constexpr size_t ST_OFF_SIGMA = 256;
+constexpr size_t ST_OFF_SECS = ST_OFF_SIGMA + sizeof(double) * DMRG_STATIC_MAX_SIGMA;
+constexpr size_t ST_OFF_PLACES = ST_OFF_SECS + sizeof(SvSector) * DMRG_STATIC_MAX_SECTORS;
+constexpr size_t ST_BYTES = ST_OFF_PLACES + sizeof(SvPlace) * DMRG_STATIC_MAX_BLOCKS;
+static_assert(ST_OFF_SECS % 256 == 0 && ST_OFF_PLACES % 256 == 0, "sub-arrays of the static scratch stay 256-byte aligned");
+static_assert(ST_BYTES <= 128 * 1024, "the static scratch is meant to stay modest");
+
+static __device__ __align__(256) unsigned char g_entropy_scratch[ST_BYTES];
+
+constexpr int ST_MAX_DEVICES = 64;
+std::mutex g_static_mu;
+unsigned char* g_static_ptr[ST_MAX_DEVICES] = {};
+
+// Device address of g_entropy_scratch on `device`, which must be the current device.
+unsigned char* static_scratch(int device) {
+  std::lock_guard<std::mutex> lk(g_static_mu);
+  DMRG_REQUIRE(device >= 0 && device < ST_MAX_DEVICES, DMRG_ERR_ARG, "bond_entropy_static: device ordinal out of range");
+  if (!g_static_ptr[device]) {
+    int cur = -1;
+    DMRG_CUDA(cudaGetDevice(&cur));
+    DMRG_REQUIRE(cur == device, DMRG_ERR_CUDA, "bond_entropy_static: the device of the context is not current");
+    void* p = nullptr;
+    DMRG_CUDA(cudaGetSymbolAddress(&p, g_entropy_scratch));
+    DMRG_REQUIRE(p != nullptr, DMRG_ERR_CUDA, "bond_entropy_static: cudaGetSymbolAddress returned a null address");
+    g_static_ptr[device] = static_cast<unsigned char*>(p);
+  }
+  return g_static_ptr[device];
+}
+
+}  // namespace
+
+extern "C" int dmrg_bond_entropy_static(dmrg_ctx* ctx, const double* d_psi, double* h_S_half, double* h_S_vn,
+                                        double* h_sigma, int32_t* n_sigma, void* stream) {
+  MO_BEGIN
+  cudaStream_t st = (cudaStream_t)stream;
+  DMRG_REQUIRE(ctx->k > 0 && d_psi, DMRG_ERR_ARG, "bond_entropy_static: no problem prepared or null pointer");
+  DMRG_REQUIRE(!ctx->su2(), DMRG_ERR_UNSUPPORTED, "bond_entropy_static: U(1)xU(1) contexts only");
+  DMRG_REQUIRE(ctx->psi.size() <= (size_t)DMRG_STATIC_MAX_BLOCKS, DMRG_ERR_UNSUPPORTED,
+               "bond_entropy_static: " + std::to_string(ctx->psi.size()) + " psi blocks exceed the static scratch (DMRG_STATIC_MAX_BLOCKS = " +
+                   std::to_string(DMRG_STATIC_MAX_BLOCKS) + "); use dmrg_bond_entropy");
+  // sectors of bond k, as in dmrg_bond_entropy: q = q_L + q(s1); rows (q_L, s1), columns (s2, q_R); lexicographic in q
+  const Sectors& SL = ctx->left->sec;
+  struct Tmp { std::map<std::pair<int, int>, int> row0, col0; int rows = 0, cols = 0; std::vector<SvPlace> pl; };
+  std::map<std::pair<int, int>, Tmp> by_q;
+  for (auto& b : ctx->psi) {
+    Tmp& t = by_q[{SL.qu[b.qL] + SITE_QU[b.s1], SL.qd[b.qL] + SITE_QD[b.s1]}];
+    auto r = t.row0.find({b.qL, b.s1});
+    if (r == t.row0.end()) { r = t.row0.emplace(std::make_pair(b.qL, b.s1), t.rows).first; t.rows += b.dL; }
+    auto c = t.col0.find({b.s2, b.qR});
+    if (c == t.col0.end()) { c = t.col0.emplace(std::make_pair(b.s2, b.qR), t.cols).first; t.cols += b.dR; }
+    t.pl.push_back(SvPlace{b.off_c, b.dL, b.dR, r->second, c->second});
+  }
+  std::vector<SvSector> secs;
+  std::vector<SvPlace> places;
+  long long nsig = 0;
+  size_t smem_max = 0;
+  for (auto& kv : by_q) {
+    Tmp& t = kv.second;
+    SvSector s{(int)places.size(), 0, t.rows, t.cols, (int)nsig, 0};
+    places.insert(places.end(), t.pl.begin(), t.pl.end());
+    s.place_end = (int)places.size();
+    const int n = std::min(t.rows, t.cols), m = std::max(t.rows, t.cols);
+    smem_max = std::max(smem_max, (size_t)n * (m + 1) * 8);
+    nsig += n;
+    secs.push_back(s);
+  }
+  // the limits of the static scratch come first: they are this entry point's own
+  DMRG_REQUIRE(nsig <= DMRG_STATIC_MAX_SIGMA, DMRG_ERR_UNSUPPORTED,
+               "bond_entropy_static: " + std::to_string(nsig) + " singular values exceed the static scratch (DMRG_STATIC_MAX_SIGMA = " +
+                   std::to_string(DMRG_STATIC_MAX_SIGMA) + "); use dmrg_bond_entropy");
+  DMRG_REQUIRE(secs.size() <= (size_t)DMRG_STATIC_MAX_SECTORS, DMRG_ERR_UNSUPPORTED,
+               "bond_entropy_static: " + std::to_string(secs.size()) + " bond sectors exceed the static scratch (DMRG_STATIC_MAX_SECTORS = " +
+                   std::to_string(DMRG_STATIC_MAX_SECTORS) + "); use dmrg_bond_entropy");
+  DMRG_REQUIRE(smem_max <= 220 * 1024, DMRG_ERR_UNSUPPORTED,
+               "bond_entropy_static: a bond sector is larger than the shared-memory Jacobi kernel holds (mode optimisation runs at D <= 256)");
+  if (n_sigma) *n_sigma = (int32_t)nsig;
+  unsigned char* base = static_scratch(ctx->cfg.device);
+  double* d_out = reinterpret_cast<double*>(base + ST_OFF_OUT);
+  double* d_sigma = reinterpret_cast<double*>(base + ST_OFF_SIGMA);
+  SvSector* d_secs = reinterpret_cast<SvSector*>(base + ST_OFF_SECS);
+  SvPlace* d_places = reinterpret_cast<SvPlace*>(base + ST_OFF_PLACES);
+  // Nothing here accumulates into the scratch: the tables are overwritten, k_sector_svals writes every sigma[0, nsig)
+  // and k_entropies all three results before anything reads them, so the previous call's contents are never seen.
+  // The results are cleared all the same, so that a kernel that failed to run cannot hand back the last call's values.
+  DMRG_CUDA(cudaMemsetAsync(d_out, 0, 256, st));
+  if (!secs.empty()) DMRG_CUDA(cudaMemcpyAsync(d_secs, secs.data(), secs.size() * sizeof(SvSector), cudaMemcpyHostToDevice, st));
+  if (!places.empty()) DMRG_CUDA(cudaMemcpyAsync(d_places, places.data(), places.size() * sizeof(SvPlace), cudaMemcpyHostToDevice, st));
+  DMRG_CUDA(cudaFuncSetAttribute(k_sector_svals, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_max));
+  if (!secs.empty()) k_sector_svals<<<(unsigned)secs.size(), 256, smem_max, st>>>(d_secs, d_places, d_psi, d_sigma);
+  k_entropies<<<1, 256, 0, st>>>(d_sigma, (int)nsig, d_out);
+  ctx->launches += 2;
+  DMRG_CUDA(cudaGetLastError());
+  double res[3];
+  DMRG_CUDA(cudaMemcpyAsync(res, d_out, sizeof(res), cudaMemcpyDeviceToHost, st));
+  if (h_sigma && nsig > 0) DMRG_CUDA(cudaMemcpyAsync(h_sigma, d_sigma, sizeof(double) * nsig, cudaMemcpyDeviceToHost, st));
+  DMRG_CUDA(cudaStreamSynchronize(st));      // the host tables above must outlive the copies
+  if (h_S_half) *h_S_half = res[0];
+  if (h_S_vn) *h_S_vn = res[1];
+  MO_END
+}
