@@ -102,6 +102,7 @@ int dmrg_load_integrals(dmrg_ctx* ctx, int32_t L, const double* h_T, const doubl
   auto V = [&](size_t i, size_t j, size_t k, size_t l) { return h_V[((i * n + j) * n + k) * n + l]; };
   for (size_t i = 0; i < n; ++i) for (size_t j = 0; j < n; ++j) for (size_t k = 0; k < n; ++k) for (size_t l = 0; l < n; ++l)
     DMRG_REQUIRE(std::fabs(V(i, j, k, l) - V(k, l, i, j)) <= 1e-12, DMRG_ERR_INPUT, "V_ijkl != V_klij");
+  ctx->drop_term_groups();                             // (waits for builders that still read the old integrals)
   ctx->T.assign(h_T, h_T + n * n);
   ctx->w.resize(n * n * n * n);
   for (size_t i = 0; i < n; ++i) for (size_t j = 0; j < n; ++j) for (size_t k = 0; k < n; ++k) for (size_t l = 0; l < n; ++l)
@@ -109,7 +110,6 @@ int dmrg_load_integrals(dmrg_ctx* ctx, int32_t L, const double* h_T, const doubl
   ctx->e_core = e_core;
   ctx->have_integrals = true;
   ctx->left_cache.clear(); ctx->right_cache.clear();   // every operator depends on the integrals
-  ctx->term_cache.clear();
   ctx->left.reset(); ctx->right.reset();
   ctx->k = 0;
   API_END

@@ -2,7 +2,9 @@
 #pragma once
 #include <cuda_runtime.h>
 
+#include <chrono>
 #include <cstdint>
+#include <cstdlib>
 #include <cstdio>
 #include <stdexcept>
 #include <string>
@@ -29,6 +31,20 @@ struct Error : std::runtime_error {
   do {                                                \
     if (!(cond)) throw dmrg::Error((code), (msg));    \
   } while (0)
+
+// DMRG_B200_TIMING=1: host-side phase times of the planning code on stderr (measurement aid)
+struct PhaseTimer {
+  bool on;
+  const char* what;
+  std::chrono::steady_clock::time_point t;
+  explicit PhaseTimer(const char* w) : on(std::getenv("DMRG_B200_TIMING") != nullptr), what(w), t(std::chrono::steady_clock::now()) {}
+  void lap(const char* name) {
+    if (!on) return;
+    auto n = std::chrono::steady_clock::now();
+    fprintf(stderr, "[timing] %s: %s %.1f ms\n", what, name, std::chrono::duration<double, std::milli>(n - t).count());
+    t = n;
+  }
+};
 
 inline int pad8(int x) { return (x + 7) & ~7; }
 

@@ -12,20 +12,6 @@
 
 namespace dmrg {
 
-// DMRG_B200_TIMING=1: host-side phase times of the planning code on stderr (measurement aid)
-struct PhaseTimer {
-  bool on;
-  const char* what;
-  std::chrono::steady_clock::time_point t;
-  explicit PhaseTimer(const char* w) : on(std::getenv("DMRG_B200_TIMING") != nullptr), what(w), t(std::chrono::steady_clock::now()) {}
-  void lap(const char* name) {
-    if (!on) return;
-    auto n = std::chrono::steady_clock::now();
-    fprintf(stderr, "[timing] %s: %s %.1f ms\n", what, name, std::chrono::duration<double, std::milli>(n - t).count());
-    t = n;
-  }
-};
-
 // ------------------------------------------------------------------------------------------------
 // class storage
 // ------------------------------------------------------------------------------------------------
@@ -556,14 +542,245 @@ static inline uint64_t pack_key4(const OpRef& l, int o1, int o2, const OpRef& r)
 // Four-part term groups of one bond: (left class, transpose, site op 1, site op 2, right class, transpose) ->
 // coefficient entries (left operator, right operator, coefficient).  They depend on the bond and the
 // integrals only, so sweeps re-use them (dmrg_ctx::term_cache).
-struct TermGroups {
+struct TermGroups : TermGroupsBase {
   struct GKey {
     int lc, lt, o1, o2, rc, rt;
     bool operator<(const GKey& o) const { return std::tie(lc, lt, o1, o2, rc, rt) < std::tie(o.lc, o.lt, o.o1, o.o2, o.rc, o.rt); }
   };
   std::map<GKey, std::vector<Entry>> groups;
-  size_t bytes() const { size_t b = 0; for (auto& kv : groups) b += kv.second.size() * sizeof(Entry); return b; }
+  size_t bytes() const override { size_t b = 0; for (auto& kv : groups) b += kv.second.size() * sizeof(Entry); return b; }
 };
+
+// Open-addressing accumulator  key -> sum of coefficients  for the term enumeration (linear probing; pack_key4 uses
+// bits 0-55 only, so ~0 marks a free slot).  Iteration is in slot order: whoever needs a fixed order sorts afterwards.
+struct FlatAcc {
+  static constexpr uint64_t FREE = ~0ull;
+  std::vector<uint64_t> keys;
+  std::vector<double> vals;
+  size_t n = 0, mask = 0;
+  explicit FlatAcc(size_t cap = 256) { keys.assign(cap, FREE); vals.assign(cap, 0.0); mask = cap - 1; }
+  static inline uint64_t mix(uint64_t x) {
+    x ^= x >> 33; x *= 0xff51afd7ed558ccdull; x ^= x >> 33; x *= 0xc4ceb9fe1a85ec53ull; x ^= x >> 33;
+    return x;
+  }
+  void grow() {
+    FlatAcc big((mask + 1) * 2);
+    for (size_t i = 0; i <= mask; ++i) if (keys[i] != FREE) big[keys[i]] = vals[i];
+    *this = std::move(big);
+  }
+  double& operator[](uint64_t key) {
+    if ((n + 1) * 10 > (mask + 1) * 7) grow();
+    size_t i = mix(key) & mask;
+    while (keys[i] != FREE && keys[i] != key) i = (i + 1) & mask;
+    if (keys[i] == FREE) { keys[i] = key; vals[i] = 0.0; ++n; }
+    return vals[i];
+  }
+  template <class F> void for_each(F&& f) const {
+    for (size_t i = 0; i <= mask; ++i) if (keys[i] != FREE) f(keys[i], vals[i]);
+  }
+};
+
+// Four-part term groups of bond k (Eq. (6)), pre-summation not yet applied: a function of (L, k, T, V) only --
+// no block data, no device work, nothing of the context written -- so it can run on a host thread ahead of the step
+// that needs it (prefetch_term_groups).
+static std::shared_ptr<TermGroups> build_term_groups(const dmrg_ctx* ctx, int k) {
+  PhaseTimer pt("term groups");
+  using GKey = TermGroups::GKey;
+  const int L = ctx->L;
+  const int o_s1 = k - 1, o_s2 = k;
+  BlockSide BL, BR;                     // for the naming of block operators only: the orbital ranges of the two blocks
+  BL.is_left = true; BL.lo = 0; BL.hi = k - 1;
+  BR.is_left = false; BR.lo = k + 1; BR.hi = L;
+  const SiteOpTable& site_ops = ctx->site_ops;   // read-only: every product of <= 4 elementary operators is interned
+  // ---- four-part terms  coef * O_L (x) o_1 (x) o_2 (x) O_R ----
+  constexpr int NB = 8;                 // buckets of the parallel enumeration = partitions of the key space
+  FlatAcc acc;
+  auto part_of = [&](int orb) { return orb < o_s1 ? 0 : (orb == o_s1 ? 1 : (orb == o_s2 ? 2 : 3)); };
+  auto add_named = [&](const OpRef& l, int o1, int o2, const OpRef& r, double coef) {
+    if (o1 < 0 || o2 < 0 || coef == 0.0) return;
+    acc[pack_key4(l, o1, o2, r)] += coef;
+  };
+  // returns false if the string cannot be named (internal error); key = 0 with c = 0 for a vanishing string
+  auto key_of = [&](const EOp* ops, int n, double coef, uint64_t& key, double& c) {
+    EOp po[4][4];
+    int np[4] = {0, 0, 0, 0}, inv = 0;
+    c = 0.0;
+    for (int i = 0; i < n; ++i) {
+      int p = part_of(ops[i].orb);
+      for (int q = p + 1; q < 4; ++q) inv += np[q];   // operators of later parts already seen
+      po[p][np[p]++] = ops[i];
+    }
+    OpRef l, r; double sl, sr;
+    int rc = name_block_ops(BL, po[0], np[0], l, sl);
+    if (rc == 1) return true;
+    if (rc != 0) return false;
+    rc = name_block_ops(BR, po[3], np[3], r, sr);
+    if (rc == 1) return true;
+    if (rc != 0) return false;
+    const int o1 = site_product(site_ops, po[1], np[1]);
+    const int o2 = site_product(site_ops, po[2], np[2]);
+    const double cc = coef * sl * sr * ((inv & 1) ? -1.0 : 1.0);
+    if (o1 < 0 || o2 < 0 || cc == 0.0) return true;
+    key = pack_key4(l, o1, o2, r);
+    c = cc;
+    return true;
+  };
+  auto add_ops = [&](const EOp* ops, int n, double coef) {
+    uint64_t key; double c;
+    DMRG_REQUIRE(key_of(ops, n, coef, key, c), DMRG_ERR_ARG, "internal: unnamed operator string");
+    if (c != 0.0) acc[key] += c;
+  };
+  const OpRef ID{K_ID, 0, false};
+  add_named(OpRef{K_H, 0, false}, 0, 0, ID, 1.0);
+  add_named(ID, 0, 0, OpRef{K_H, 0, false}, 1.0);
+  for (int s = 0; s < 2; ++s) {
+    const EOp ec{true, 0, s}, ea{false, 0, s};
+    const int oc_ = site_product(site_ops, &ec, 1), oa_ = site_product(site_ops, &ea, 1);
+    const int sk = s == 0 ? K_SU : K_SD, ck = s == 0 ? K_CU : K_CD;
+    // x outside L:  a+_x S^L_x = - S^L_x a+_x ,  h.c. = (S^L_x)^T a_x
+    for (int x = o_s1; x < L; ++x) {
+      OpRef S{sk, idx_S(BL, x), false}, St{sk, idx_S(BL, x), true};
+      if (x == o_s1) { add_named(S, oc_, 0, ID, -1.0); add_named(St, oa_, 0, ID, 1.0); }
+      else if (x == o_s2) { add_named(S, 0, oc_, ID, -1.0); add_named(St, 0, oa_, ID, 1.0); }
+      else { add_named(S, 0, 0, OpRef{ck, x - BR.lo, false}, -1.0); add_named(St, 0, 0, OpRef{ck, x - BR.lo, true}, 1.0); }
+    }
+    // x outside R:  a+_x S^R_x ,  h.c. = (S^R_x)^T a_x = - a_x (S^R_x)^T
+    for (int x = 0; x <= o_s2; ++x) {
+      OpRef S{sk, idx_S(BR, x), false}, St{sk, idx_S(BR, x), true};
+      if (x == o_s1) { add_named(ID, oc_, 0, S, 1.0); add_named(ID, oa_, 0, St, -1.0); }
+      else if (x == o_s2) { add_named(ID, 0, oc_, S, 1.0); add_named(ID, 0, oa_, St, -1.0); }
+      else { add_named(OpRef{ck, x - BL.lo, false}, 0, 0, S, 1.0); add_named(OpRef{ck, x - BL.lo, true}, 0, 0, St, -1.0); }
+    }
+  }
+  auto is_block = [&](int p) { return p == 0 || p == 3; };
+  for (int i = 0; i < L; ++i) for (int j = 0; j < L; ++j) {
+    int pi = part_of(i), pj = part_of(j);
+    if (pi == pj && is_block(pi)) continue;                        // inside H^L / H^R
+    double f = 1.0;
+    if (pi != pj) f -= 0.5 * (is_block(pi) ? 1 : 0) + 0.5 * (is_block(pj) ? 1 : 0);   // halves carried by S^L, S^R
+    double tv = f * T2(ctx, i, j);
+    if (tv == 0.0) continue;
+    for (int s = 0; s < 2; ++s) {
+      EOp o[2] = {{true, i, s}, {false, j, s}};
+      add_ops(o, 2, tv);
+    }
+  }
+  pt.lap("one-body + S strings");
+  // The L^4 two-body strings: NB buckets (i mod NB), each with one private map per key partition (key mod NB), filled
+  // in parallel; partition p then sums its maps in bucket order, so the coefficient sums do not depend on the
+  // number of threads.
+  std::vector<FlatAcc> loc((size_t)NB * NB);
+  std::vector<FlatAcc> parts(NB);
+  {
+    int err_any = 0;
+#pragma omp parallel for num_threads(NB) schedule(static, 1)
+    for (int b = 0; b < NB; ++b) {
+      int err = 0;
+      FlatAcc* mine = &loc[(size_t)b * NB];
+      for (int i = b; i < L; i += NB)
+        for (int j = 0; j < L; ++j) for (int kk = 0; kk < L; ++kk) for (int l = 0; l < L; ++l) {
+          int cnt[4] = {0, 0, 0, 0};
+          ++cnt[part_of(i)]; ++cnt[part_of(j)]; ++cnt[part_of(kk)]; ++cnt[part_of(l)];
+          if (cnt[0] >= 3 || cnt[3] >= 3) continue;                      // inside H^L/H^R or a+ S + h.c.
+          const double wv = 0.5 * W4(ctx, i, j, kk, l);
+          if (wv == 0.0) continue;
+          for (int s = 0; s < 2; ++s) for (int t = 0; t < 2; ++t) {
+            EOp o[4] = {{true, i, s}, {true, j, t}, {false, l, t}, {false, kk, s}};
+            uint64_t key; double c;
+            if (!key_of(o, 4, wv, key, c)) { err = 1; continue; }
+            if (c != 0.0) mine[key % NB][key] += c;
+          }
+        }
+      if (err) {
+#pragma omp atomic write
+        err_any = 1;
+      }
+    }
+    DMRG_REQUIRE(!err_any, DMRG_ERR_ARG, "internal: unnamed operator string");
+    pt.lap("two-body strings (parallel)");
+#pragma omp parallel for num_threads(NB) schedule(static, 1)
+    for (int p = 0; p < NB; ++p) {
+      FlatAcc& out = parts[p];
+      acc.for_each([&](uint64_t key, double v) { if ((int)(key % NB) == p) out[key] += v; });   // one-body, S, H strings
+      for (int b = 0; b < NB; ++b) loc[(size_t)b * NB + p].for_each([&](uint64_t key, double v) { out[key] += v; });
+    }
+    loc.clear();
+  }
+  pt.lap("merge");
+  // ---- group the terms by (left class, transpose, site operators, right class, transpose) ----
+  auto tg = std::make_shared<TermGroups>();
+  std::map<GKey, std::vector<Entry>>& groups = tg->groups;   // Entry: a = left index, b = right index
+  {
+    std::unordered_map<uint64_t, std::vector<Entry>*> fast;   // group bits of the key -> its entry list
+    const uint64_t gmask = ~((0xFFFull << 38) | (0xFFFull << 1));
+    for (auto& part : parts)
+      part.for_each([&](uint64_t q, double v) {
+        if (std::fabs(v) < 1e-300) return;
+        std::vector<Entry>*& e = fast[q & gmask];
+        if (!e) {
+          GKey g{(int)(q >> 50) & 63, (int)(q >> 37) & 1, (int)(q >> 28) & 511, (int)(q >> 19) & 511,
+                 (int)(q >> 13) & 63, (int)(q & 1)};
+          e = &groups[g];
+        }
+        e->push_back(Entry{(int)(q >> 38) & 4095, (int)(q >> 1) & 4095, v});
+      });
+    // a fixed entry order inside every group (the maps iterate in slot order)
+    std::vector<std::vector<Entry>*> gv;
+    for (auto& kv : groups) gv.push_back(&kv.second);
+#pragma omp parallel for num_threads(NB) schedule(dynamic, 1)
+    for (int g = 0; g < (int)gv.size(); ++g)
+      std::sort(gv[g]->begin(), gv[g]->end(), [](const Entry& x, const Entry& y) { return x.a != y.a ? x.a < y.a : x.b < y.b; });
+  }
+  pt.lap("group");
+  return tg;
+}
+
+static void cache_term_groups(dmrg_ctx* ctx, int k, const std::shared_ptr<TermGroupsBase>& tg) {
+  size_t cached = 0;
+  for (auto& kv : ctx->term_cache) cached += kv.second->bytes();
+  if (cached + tg->bytes() <= (size_t)1 << 30) ctx->term_cache[k] = tg;   // host memory cap: 1 GiB
+}
+
+static std::shared_ptr<TermGroupsBase> build_term_groups_su2(const dmrg_ctx* ctx, int k);   // engine_su2.inc
+
+// Starts building the term groups of bond k on a host thread unless they are cached or on their way.  Called when a
+// two-site problem has been prepared, for its two neighbours: a sweep needs one of them next, and the build (an
+// O(L^4) enumeration) then runs while the eigensolver keeps the GPU busy instead of in front of the next step
+// ("Tables": host work that should not show up in the sweep time).  DMRG_B200_NO_PREFETCH=1 turns it off.
+static void prefetch_term_groups(dmrg_ctx* ctx, int k) {
+  static const bool off = std::getenv("DMRG_B200_NO_PREFETCH") != nullptr;
+  if (off || k < 1 || k + 1 > ctx->L || ctx->term_cache.count(k) || ctx->term_prefetch.count(k)) return;
+  const dmrg_ctx* c = ctx;
+  ctx->term_prefetch[k] = std::async(std::launch::async, [c, k]() -> std::shared_ptr<TermGroupsBase> {
+                            if (c->su2()) return build_term_groups_su2(c, k);
+                            return build_term_groups(c, k);
+                          }).share();
+}
+
+static void harvest_term_prefetch(dmrg_ctx* ctx);
+static void prefetch_neighbour_term_groups(dmrg_ctx* ctx) {
+  harvest_term_prefetch(ctx);
+  prefetch_term_groups(ctx, ctx->k + 1);
+  prefetch_term_groups(ctx, ctx->k - 1);
+}
+
+// The term groups of bond k if a host thread is building (or has built) them; waits for it.  Null if none is.
+static std::shared_ptr<TermGroupsBase> take_prefetched_term_groups(dmrg_ctx* ctx, int k) {
+  auto pf = ctx->term_prefetch.find(k);
+  if (pf == ctx->term_prefetch.end()) return nullptr;
+  auto fut = pf->second;
+  ctx->term_prefetch.erase(pf);
+  return fut.get();     // (rethrows what the builder threw)
+}
+
+// Moves finished builds into the cache (the ones of the direction the sweep did not take).
+static void harvest_term_prefetch(dmrg_ctx* ctx) {
+  for (auto it = ctx->term_prefetch.begin(); it != ctx->term_prefetch.end();) {
+    if (it->second.wait_for(std::chrono::seconds(0)) != std::future_status::ready) { ++it; continue; }
+    try { cache_term_groups(ctx, it->first, it->second.get()); } catch (...) {}   // (a failed build is simply not cached)
+    it = ctx->term_prefetch.erase(it);
+  }
+}
 
 // Output-block sharding of H_eff.psi over ranks ("independent operations"): every psi'
 // block is computed completely by one rank, so the exchange is a sum with exact zeros.  Longest-processing-time
@@ -626,11 +843,11 @@ static void finish_superblock(dmrg_ctx* ctx, std::vector<std::vector<DiagTask>>&
 
 
 void prepare_superblock(dmrg_ctx* ctx, cudaStream_t st) {
-  const int L = ctx->L, k = ctx->k;
+  const int k = ctx->k;
   BlockSide& BL = *ctx->left;
   BlockSide& BR = *ctx->right;
-  DMRG_REQUIRE(BL.hi == k - 1 && BR.lo == k + 1, DMRG_ERR_ARG, "superblock: environments do not match the bond");
-  const int o_s1 = k - 1, o_s2 = k;
+  DMRG_REQUIRE(BL.lo == 0 && BL.hi == k - 1 && BR.lo == k + 1 && BR.hi == ctx->L, DMRG_ERR_ARG,
+               "superblock: environments do not match the bond");
   const int NU = ctx->cfg.n_up, ND = ctx->cfg.n_dn;
   // drop pre-summed classes of an earlier bond
   BL.cls.resize(K_NSTD);
@@ -677,146 +894,15 @@ void prepare_superblock(dmrg_ctx* ctx, cudaStream_t st) {
     if (f != ctx->term_cache.end()) tg = std::static_pointer_cast<TermGroups>(f->second);
   }
   if (!tg) {
-    // ---- four-part terms  coef * O_L (x) o_1 (x) o_2 (x) O_R  of PAPER.md Eq. (6) ----
-    std::unordered_map<uint64_t, double> acc;
-    auto part_of = [&](int orb) { return orb < o_s1 ? 0 : (orb == o_s1 ? 1 : (orb == o_s2 ? 2 : 3)); };
-    auto add_named = [&](const OpRef& l, int o1, int o2, const OpRef& r, double coef) {
-      if (o1 < 0 || o2 < 0 || coef == 0.0) return;
-      acc[pack_key4(l, o1, o2, r)] += coef;
-    };
-    using AccMap = std::unordered_map<uint64_t, double>;
-    std::vector<AccMap> parts;
-    auto add_ops_to = [&](AccMap& m, const EOp* ops, int n, double coef, int* err) {
-      EOp po[4][4];
-      int np[4] = {0, 0, 0, 0}, inv = 0;
-      for (int i = 0; i < n; ++i) {
-        int p = part_of(ops[i].orb);
-        for (int q = p + 1; q < 4; ++q) inv += np[q];   // operators of later parts already seen
-        po[p][np[p]++] = ops[i];
-      }
-      OpRef l, r; double sl, sr;
-      int rc = name_block_ops(BL, po[0], np[0], l, sl);
-      if (rc == 1) return;
-      if (rc != 0) { *err = 1; return; }
-      rc = name_block_ops(BR, po[3], np[3], r, sr);
-      if (rc == 1) return;
-      if (rc != 0) { *err = 1; return; }
-      const int o1 = site_product(ctx->site_ops, po[1], np[1]);
-      const int o2 = site_product(ctx->site_ops, po[2], np[2]);
-      const double c = coef * sl * sr * ((inv & 1) ? -1.0 : 1.0);
-      if (o1 < 0 || o2 < 0 || c == 0.0) return;
-      m[pack_key4(l, o1, o2, r)] += c;
-    };
-    auto add_ops = [&](const EOp* ops, int n, double coef) {
-      int err = 0;
-      add_ops_to(acc, ops, n, coef, &err);
-      DMRG_REQUIRE(!err, DMRG_ERR_ARG, "internal: unnamed operator string");
-    };
-    const OpRef ID{K_ID, 0, false};
-    add_named(OpRef{K_H, 0, false}, 0, 0, ID, 1.0);
-    add_named(ID, 0, 0, OpRef{K_H, 0, false}, 1.0);
-    for (int s = 0; s < 2; ++s) {
-      double mc[16], ma[16];
-      site_elem(true, s, mc);
-      site_elem(false, s, ma);
-      const int oc_ = ctx->site_ops.intern(mc), oa_ = ctx->site_ops.intern(ma);
-      const int sk = s == 0 ? K_SU : K_SD, ck = s == 0 ? K_CU : K_CD;
-      // x outside L:  a+_x S^L_x = - S^L_x a+_x ,  h.c. = (S^L_x)^T a_x
-      for (int x = o_s1; x < L; ++x) {
-        OpRef S{sk, idx_S(BL, x), false}, St{sk, idx_S(BL, x), true};
-        if (x == o_s1) { add_named(S, oc_, 0, ID, -1.0); add_named(St, oa_, 0, ID, 1.0); }
-        else if (x == o_s2) { add_named(S, 0, oc_, ID, -1.0); add_named(St, 0, oa_, ID, 1.0); }
-        else { add_named(S, 0, 0, OpRef{ck, x - BR.lo, false}, -1.0); add_named(St, 0, 0, OpRef{ck, x - BR.lo, true}, 1.0); }
-      }
-      // x outside R:  a+_x S^R_x ,  h.c. = (S^R_x)^T a_x = - a_x (S^R_x)^T
-      for (int x = 0; x <= o_s2; ++x) {
-        OpRef S{sk, idx_S(BR, x), false}, St{sk, idx_S(BR, x), true};
-        if (x == o_s1) { add_named(ID, oc_, 0, S, 1.0); add_named(ID, oa_, 0, St, -1.0); }
-        else if (x == o_s2) { add_named(ID, 0, oc_, S, 1.0); add_named(ID, 0, oa_, St, -1.0); }
-        else { add_named(OpRef{ck, x - BL.lo, false}, 0, 0, S, 1.0); add_named(OpRef{ck, x - BL.lo, true}, 0, 0, St, -1.0); }
-      }
+    auto got = take_prefetched_term_groups(ctx, k);
+    if (got) {
+      tg = std::static_pointer_cast<TermGroups>(got);
+      pt.lap("term groups from the prefetch thread");
+    } else {
+      tg = build_term_groups(ctx, k);
+      pt.lap("term groups built here");
     }
-    auto is_block = [&](int p) { return p == 0 || p == 3; };
-    for (int i = 0; i < L; ++i) for (int j = 0; j < L; ++j) {
-      int pi = part_of(i), pj = part_of(j);
-      if (pi == pj && is_block(pi)) continue;                        // inside H^L / H^R
-      double f = 1.0;
-      if (pi != pj) f -= 0.5 * (is_block(pi) ? 1 : 0) + 0.5 * (is_block(pj) ? 1 : 0);   // halves carried by S^L, S^R
-      double tv = f * T2(ctx, i, j);
-      if (tv == 0.0) continue;
-      for (int s = 0; s < 2; ++s) {
-        EOp o[2] = {{true, i, s}, {false, j, s}};
-        add_ops(o, 2, tv);
-      }
-    }
-    pt.lap("one-body + S strings");
-    // The L^4 two-body strings: eight buckets (i mod 8) with private maps, processed in parallel and merged
-    // in bucket order, so the coefficient sums do not depend on the number of threads.
-    {
-      constexpr int NB = 8;
-      std::vector<AccMap> loc(NB);
-      int err_any = 0;
-  #pragma omp parallel for num_threads(NB) schedule(static, 1)
-      for (int b = 0; b < NB; ++b) {
-        int err = 0;
-        for (int i = b; i < L; i += NB)
-          for (int j = 0; j < L; ++j) for (int kk = 0; kk < L; ++kk) for (int l = 0; l < L; ++l) {
-            int cnt[4] = {0, 0, 0, 0};
-            ++cnt[part_of(i)]; ++cnt[part_of(j)]; ++cnt[part_of(kk)]; ++cnt[part_of(l)];
-            if (cnt[0] >= 3 || cnt[3] >= 3) continue;                      // inside H^L/H^R or a+ S + h.c.
-            const double wv = 0.5 * W4(ctx, i, j, kk, l);
-            if (wv == 0.0) continue;
-            for (int s = 0; s < 2; ++s) for (int t = 0; t < 2; ++t) {
-              EOp o[4] = {{true, i, s}, {true, j, t}, {false, l, t}, {false, kk, s}};
-              add_ops_to(loc[b], o, 4, wv, &err);
-            }
-          }
-        if (err) {
-  #pragma omp atomic write
-          err_any = 1;
-        }
-      }
-      DMRG_REQUIRE(!err_any, DMRG_ERR_ARG, "internal: unnamed operator string");
-      pt.lap("two-body strings (parallel)");
-      // merge: partition p takes the keys with key % NB == p from every bucket map, in bucket order
-      parts.resize(NB);
-  #pragma omp parallel for num_threads(NB) schedule(static, 1)
-      for (int p = 0; p < NB; ++p) {
-        AccMap& out = parts[p];
-        for (auto& kv : acc) if ((int)(kv.first % NB) == p) out[kv.first] += kv.second;   // one-body, S, H strings
-        for (int b = 0; b < NB; ++b)
-          for (auto& kv : loc[b]) if ((int)(kv.first % NB) == p) out[kv.first] += kv.second;
-      }
-    }
-    pt.lap("merge");
-    // ---- group terms; pre-sum one side into complementary operators where that shortens the list ----
-    std::map<GKey, std::vector<Entry>> groups;   // Entry: a = left index, b = right index
-    {
-      std::unordered_map<uint64_t, std::vector<Entry>*> fast;   // group bits of the key -> its entry list
-      const uint64_t gmask = ~((0xFFFull << 38) | (0xFFFull << 1));
-      for (auto& part : parts)
-        for (auto& kv : part) {
-          if (std::fabs(kv.second) < 1e-300) continue;
-          const uint64_t q = kv.first;
-          std::vector<Entry>*& v = fast[q & gmask];
-          if (!v) {
-            GKey g{(int)(q >> 50) & 63, (int)(q >> 37) & 1, (int)(q >> 28) & 511, (int)(q >> 19) & 511,
-                   (int)(q >> 13) & 63, (int)(q & 1)};
-            v = &groups[g];
-          }
-          v->push_back(Entry{(int)(q >> 38) & 4095, (int)(q >> 1) & 4095, kv.second});
-        }
-      // a fixed entry order inside every group (the partition maps iterate in hash order)
-      for (auto& kv : groups)
-        std::sort(kv.second.begin(), kv.second.end(), [](const Entry& x, const Entry& y) { return x.a != y.a ? x.a < y.a : x.b < y.b; });
-    }
-    parts.clear();
-    acc.clear();
-    tg = std::make_shared<TermGroups>();
-    tg->groups = std::move(groups);
-    size_t cached = 0;
-    for (auto& kv : ctx->term_cache) cached += std::static_pointer_cast<TermGroups>(kv.second)->bytes();
-    if (cached + tg->bytes() <= (size_t)1 << 30) ctx->term_cache[k] = tg;   // host memory cap: 1 GiB
+    cache_term_groups(ctx, k, tg);
   } else {
     pt.lap("term groups from cache");
   }
@@ -857,8 +943,9 @@ void prepare_superblock(dmrg_ctx* ctx, cudaStream_t st) {
     n_terms += (int64_t)f.e.size();
     fgs.push_back(std::move(f));
   }
+  pt.lap("pre-sum: coefficient matrices, classes, items");
   pre.run();
-  pt.lap("group + pre-sum");
+  pt.lap("pre-sum: plan + launches + sync");
 
   // ---- tasks of PAPER.md Eq. (8): (term group x psi block) -> contraction items + diagonal tasks ----
   const uint64_t cap = workspace_cap(ctx);
@@ -965,6 +1052,8 @@ void prepare_superblock(dmrg_ctx* ctx, cudaStream_t st) {
   pt.lap("planner.finish");
   finish_superblock(ctx, dtasks, n_terms, n_tasks, n_groups, st);
   pt.lap("diag + stats");
+  // the sweep goes to one of the neighbouring bonds next: their term groups are built while the eigensolver runs
+  prefetch_neighbour_term_groups(ctx);
 }
 
 #include "engine_su2.inc"

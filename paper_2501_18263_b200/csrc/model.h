@@ -7,6 +7,7 @@
 // so that "one block of every operator in a term group" is a strided batch for the GEMM kernel.
 #pragma once
 #include <array>
+#include <future>
 #include <map>
 #include <memory>
 
@@ -110,6 +111,12 @@ struct SiteOpTable {
   int parity(int id) const;
 };
 
+// Term groups of the two-site problem of one bond (engine.cu, engine_su2.inc): a function of the bond and the integrals.
+struct TermGroupsBase {
+  virtual ~TermGroupsBase() = default;
+  virtual size_t bytes() const = 0;
+};
+
 struct PsiBlk { int qL, s1, s2, qR; int dL, dR, dLp, dRp; long long off_c, off_p; int qLp = -1; /* SU(2): (N, 2S) of L' */ int NLp = 0, SLp = 0; };
 
 }  // namespace dmrg
@@ -130,7 +137,16 @@ struct dmrg_ctx {
   // environment cache for sweeps: left_cache[i] = block of sites 1..i, right_cache[i] = block of sites i..L.
   // Entries are dropped when a site tensor or bond they depend on changes; total size is capped.
   std::map<int, std::shared_ptr<dmrg::BlockSide>> left_cache, right_cache;
-  std::map<int, std::shared_ptr<void>> term_cache;   // bond k -> term groups of the two-site problem (engine.cu)
+  std::map<int, std::shared_ptr<dmrg::TermGroupsBase>> term_cache;   // bond k -> term groups of the two-site problem
+  // Term groups of neighbouring bonds being built ahead of time on host threads (engine.cu prefetch_term_groups).
+  // The builders read L, T, w and site_ops: whoever changes those calls drop_term_groups() first.
+  std::map<int, std::shared_future<std::shared_ptr<dmrg::TermGroupsBase>>> term_prefetch;
+  void drop_term_groups() {
+    for (auto& kv : term_prefetch) if (kv.second.valid()) kv.second.wait();
+    term_prefetch.clear();
+    term_cache.clear();
+  }
+  ~dmrg_ctx() { for (auto& kv : term_prefetch) if (kv.second.valid()) kv.second.wait(); }
   std::shared_ptr<dmrg::HostPool> host_pool;         // host tier (cfg.env_host_bytes > 0)
   int64_t n_spills = 0, n_fetches = 0;
   uint64_t cache_bytes() const {      // device-resident bytes of the cached blocks

@@ -307,6 +307,7 @@ int dmrg_rotate_integrals(dmrg_ctx* ctx, int32_t k, double theta) {
   DMRG_REQUIRE(ctx->have_integrals && k >= 1 && k + 1 <= ctx->L, DMRG_ERR_ARG, "rotate_integrals: integrals first, 1 <= k < L");
   const size_t n = (size_t)ctx->L, a = (size_t)k - 1, b = (size_t)k;
   const double c = std::cos(theta), s = std::sin(theta);
+  ctx->drop_term_groups();              // (waits for builders that still read the old integrals)
   // new orbital a~ = c a + s b, b~ = -s a + c b (creation operators transform with the same matrix): every index of
   // T and w is rotated in turn
   auto rot = [&](std::vector<double>& t, int rank) {
@@ -326,7 +327,6 @@ int dmrg_rotate_integrals(dmrg_ctx* ctx, int32_t k, double theta) {
   rot(ctx->w, 4);
   // every operator of every block depends on the integrals
   ctx->left_cache.clear(); ctx->right_cache.clear();
-  ctx->term_cache.clear();
   ctx->left.reset(); ctx->right.reset();
   ctx->apply_plan.clear();
   ctx->k = 0;

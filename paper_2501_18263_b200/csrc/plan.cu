@@ -388,6 +388,7 @@ void Planner::add_piece(const Item& it, int b0, int cnt) {
 }
 
 void Planner::finish(Plan* plan, cudaStream_t st) {
+  PhaseTimer pt("  planner.finish");
   plan->clear();
   plan->flops_analytic = fa_;
   plan->flops_executed = fe_;
@@ -483,6 +484,7 @@ void Planner::finish(Plan* plan, cudaStream_t st) {
     hv.swap(ex);
     scratch_max = std::max(scratch_max, sc_used);
   }
+  pt.lap("split-K");
   // ---- fused small-sector outputs: tile class, split of heavy task lists into parts, launch order ----
   struct FPart { int out; bool partial; long long sc_off; std::vector<FTask> tasks; double cost; int cls; };
   std::vector<FPart> fparts;
@@ -547,6 +549,7 @@ void Planner::finish(Plan* plan, cudaStream_t st) {
     }
     scratch_max = std::max(scratch_max, fsc_used);
   }
+  pt.lap("fused parts");
   if (scratch_max > 0) plan->scratch.allocate(al_, (size_t)scratch_max);
   double* sc = plan->scratch.p;
   if (!fparts.empty()) {
@@ -645,6 +648,7 @@ void Planner::finish(Plan* plan, cudaStream_t st) {
     ph.outs.upload(al_, outs, st);
     ph.segs.upload(al_, segs, st);
   };
+  pt.lap("fused upload");
   plan->chunks.resize(chunks_.size());
   struct PS { double act = 0, full = 0; long long tiles = 0; } ps[2][GEMM_NSHAPES];
   for (size_t c = 0; c < chunks_.size(); ++c) {
@@ -679,7 +683,9 @@ void Planner::finish(Plan* plan, cudaStream_t st) {
           fprintf(stderr, "plan phase %d shape %dx%d tiles %lld flops %.4g full-tile flops %.4g (fill %.3f)\n", p + 1,
                   GEMM_DIMS[sh / 3], GEMM_DIMS[sh % 3], ps[p][sh].tiles, ps[p][sh].act, ps[p][sh].full,
                   ps[p][sh].act / ps[p][sh].full);
+  pt.lap("chunk tile lists + upload");
   chunks_.clear();
+  pt.lap("free host items");
 }
 
 }  // namespace dmrg
