@@ -222,6 +222,37 @@ int dmrg_rotate_integrals(dmrg_ctx* ctx, int32_t k, double theta);
 int dmrg_bond_entropy_static(dmrg_ctx* ctx, const double* d_psi, double* h_S_half, double* h_S_vn, double* h_sigma,
                              int32_t* n_sigma, void* stream);
 
+/* ---- truncation step of a micro-iteration ("keeping only the D largest singular values in SVD"; Fig. 1
+ * :63 "SVD"; the "SVD" and "StVec" columns of the paper's timing table :284); U(1)xU(1) ----
+ *
+ * dmrg_truncate_bond: d_psi (device, read only) is the optimised two-site wavefunction of the prepared problem at bond
+ * (k, k+1).  Psi[(a s_k), (s_{k+1} b)] is decomposed per sector of bond k by a one-sided Jacobi SVD on the device;
+ * the D largest singular values over all sectors are kept (values <= 1e-14 never; equal values: the sector that comes
+ * first in lexicographic (n_up, n_dn) order first, R23).  The library then replaces its sectors of bond k by
+ * the kept ones and installs, without a host round trip, the new left-canonical tensor of site k (direction 0, the
+ * sweep moves right: A = U) or the new right-canonical tensor of site k+1 (direction 1: B = V^T); the tensor of the
+ * other centre site becomes unset and cached environment blocks that contain either site are dropped, exactly as
+ * dmrg_mps_update_bond + dmrg_mps_set_site would do.  The prepared problem stays prepared: call
+ * dmrg_renormalize(direction) next.  *h_discarded = sum of the squares of the singular values not among the D largest;
+ * *h_kept = number of kept states (both host, optional).
+ *   The Jacobi kernel holds a sector matrix in the shared memory of one CTA when rows x columns <= ~27 000 (~165 x 165:
+ * bond dimensions up to D ~ 256, the regime of the paper's mode optimisation); a larger sector is rotated in place in
+ * global memory, which is correct at any size but slow (a caller at large D may prefer its own SVD with
+ * dmrg_mps_update_bond / dmrg_mps_set_site).  DMRG_ERR_UNSUPPORTED for SU(2) contexts (nothing changed then).
+ * Synchronises `stream`.
+ *
+ * dmrg_start_vector: after dmrg_truncate_bond(direction) and dmrg_renormalize(direction), d_psi_out (device,
+ * dmrg_psi_layout of the NEW problem) receives the wave-function transformation of the truncated state: the centre
+ * factor Sigma V^T (or U Sigma) contracted with the canonical tensor of the site that joined the two-site centre.  Not
+ * normalised.  DMRG_ERR_ARG if the calls did not come in that order.  Synchronises `stream`.
+ *
+ * dmrg_bond_sectors: the sectors of bond b (0..L) as the library holds them, in lexicographic order; *nsec always,
+ * the arrays (host, capacity >= *nsec, any may be NULL) when given. */
+int dmrg_truncate_bond(dmrg_ctx* ctx, const double* d_psi, int32_t direction, int32_t D, double* h_discarded,
+                       int32_t* h_kept, void* stream);
+int dmrg_start_vector(dmrg_ctx* ctx, double* d_psi_out, void* stream);
+int dmrg_bond_sectors(dmrg_ctx* ctx, int32_t b, int32_t* nsec, int32_t* h_q_up, int32_t* h_q_dn, int32_t* h_dim);
+
 typedef struct {
   int64_t n_terms;          /* four-part terms of PAPER.md Eq. (6) after pre-summation */
   int64_t n_tasks;          /* (term x sector) tasks of PAPER.md Eq. (8) */

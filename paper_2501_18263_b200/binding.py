@@ -24,6 +24,7 @@ EXPORTS = [
     "dmrg_env_export", "dmrg_fp64_peak", "dmrg_apply_profile", "dmrg_mps_set_site_su2", "dmrg_su2_f_factor",
     "dmrg_mps_update_bond", "dmrg_set_shard", "dmrg_shard_info", "dmrg_env_export_block", "dmrg_block_flops", "dmrg_dfma_peak",
     "dmrg_two_site_gate", "dmrg_bond_entropy", "dmrg_rotate_integrals", "dmrg_rotation_gate", "dmrg_bond_entropy_static",
+    "dmrg_truncate_bond", "dmrg_start_vector", "dmrg_bond_sectors",
 ]
 
 STATIC_MAX_SIGMA, STATIC_MAX_SECTORS, STATIC_MAX_BLOCKS = 2048, 512, 4096     # include/dmrg_b200.h DMRG_STATIC_MAX_*
@@ -106,6 +107,9 @@ def load_library(build_if_missing: bool = True):
     lib.dmrg_two_site_gate.argtypes = [vp, vp, vp, vp, vp]
     lib.dmrg_bond_entropy.argtypes = [vp, vp, dp, dp, vp, C.POINTER(i32), vp]
     lib.dmrg_bond_entropy_static.argtypes = [vp, vp, dp, dp, vp, C.POINTER(i32), vp]
+    lib.dmrg_truncate_bond.argtypes = [vp, vp, i32, i32, dp, C.POINTER(i32), vp]
+    lib.dmrg_start_vector.argtypes = [vp, vp, vp]
+    lib.dmrg_bond_sectors.argtypes = [vp, i32, C.POINTER(i32), vp, vp, vp]
     lib.dmrg_rotate_integrals.argtypes = [vp, i32, C.c_double]
     lib.dmrg_rotation_gate.argtypes = [C.c_double, vp]
     lib.dmrg_apply_profile.argtypes = [vp, vp, vp, i32, C.POINTER(LaunchInfo), C.POINTER(i32), vp]
@@ -390,6 +394,30 @@ class DMRG:
         self._check(self.lib.dmrg_bond_entropy_static(self.ctx, C.c_void_p(psi.data_ptr()), C.byref(a), C.byref(b),
                                                       _np_ptr(sig) if spectrum else None, C.byref(n), self._stream()))
         return (a.value, b.value, sig[:n.value]) if spectrum else (a.value, b.value)
+
+    def truncate_bond(self, psi, direction, D):
+        """SVD truncation of the optimised two-site wavefunction psi inside the library (dmrg_truncate_bond): new
+        sectors of bond k and the new canonical site tensor are installed on the device.  Returns (discarded weight,
+        number of kept states).  Call renormalize(direction) next, then start_vector()."""
+        w, n = C.c_double(), C.c_int32()
+        self._check(self.lib.dmrg_truncate_bond(self.ctx, C.c_void_p(psi.data_ptr()), int(direction), int(D), C.byref(w),
+                                                C.byref(n), self._stream()))
+        return w.value, n.value
+
+    def start_vector(self, out=None):
+        """The truncated state in the layout of the problem prepared by renormalize (dmrg_start_vector); not normalised."""
+        if out is None:
+            out = self.torch.empty(self.psi_size(), dtype=self.torch.float64, device=self.device)
+        self._check(self.lib.dmrg_start_vector(self.ctx, C.c_void_p(out.data_ptr()), self._stream()))
+        return out
+
+    def bond_sectors(self, b):
+        """dict (n_up, n_dn) -> dimension of bond b as the library holds it."""
+        n = C.c_int32()
+        self._check(self.lib.dmrg_bond_sectors(self.ctx, int(b), C.byref(n), None, None, None))
+        a = [np.zeros(max(n.value, 1), dtype=np.int32) for _ in range(3)]
+        self._check(self.lib.dmrg_bond_sectors(self.ctx, int(b), C.byref(n), *[_np_ptr(x) for x in a]))
+        return {(int(a[0][i]), int(a[1][i])): int(a[2][i]) for i in range(n.value)}
 
     def rotate_integrals(self, k, theta):
         self._check(self.lib.dmrg_rotate_integrals(self.ctx, int(k), float(theta)))

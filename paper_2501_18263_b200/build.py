@@ -8,7 +8,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libdmrg_b200.so")
-SOURCES = ["gemm.cu", "fused.cu", "kernels.cu", "plan.cu", "su2.cu", "engine.cu", "api.cu", "modeopt.cu"]
+SOURCES = ["gemm.cu", "fused.cu", "kernels.cu", "plan.cu", "su2.cu", "engine.cu", "api.cu", "modeopt.cu", "truncate.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC,-fopenmp"]
 

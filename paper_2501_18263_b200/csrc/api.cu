@@ -139,6 +139,7 @@ int dmrg_mps_set_sectors(dmrg_ctx* ctx, const int32_t* off, const int32_t* qu, c
     DMRG_REQUIRE(bond[L].size() == 1 && bond[L].qu[0] == ctx->cfg.n_up && bond[L].qd[0] == ctx->cfg.n_dn &&
                      bond[L].dim[0] == 1, DMRG_ERR_INPUT, "set_sectors: bond L must be {(n_up,n_dn):1}");
   ctx->bond = std::move(bond);
+  ctx->centre.clear();
   for (auto& s : ctx->site) { s.canonical = -1; s.blks.clear(); s.find.clear(); s.find3.clear(); s.data.release(); }
   ctx->left_cache.clear(); ctx->right_cache.clear();
   ctx->left.reset(); ctx->right.reset();
@@ -247,6 +248,7 @@ int dmrg_mps_update_bond(dmrg_ctx* ctx, int32_t b, int32_t nsec, const int32_t* 
     s.add(qu[i], qd[i], dim[i]);
   }
   ctx->bond[b] = std::move(s);
+  ctx->centre.clear();                      // (a centre factor of dmrg_truncate_bond refers to the old sectors)
   for (int i : {b, b + 1}) {
     SiteTensor& t = ctx->site[i];
     t.canonical = -1; t.blks.clear(); t.find.clear(); t.find3.clear(); t.data.release();

@@ -117,6 +117,21 @@ struct TermGroupsBase {
   virtual size_t bytes() const = 0;
 };
 
+// What dmrg_truncate_bond leaves behind for dmrg_start_vector (truncate.cu): per kept sector of the truncated bond the
+// centre factor, c rows in descending order of the singular values: Sigma V^T (row length = columns of the sector) when
+// the sweep moves right, (U Sigma)^T (row length = rows of the sector) when it moves left.
+struct CentreFactor {
+  int bond = 0, direction = -1;            // bond == 0: none
+  DevArray<double> C;
+  struct Sec {
+    int c = 0, len = 0;                    // kept states, row length
+    long long off = 0;                     // first element in C
+    std::map<std::pair<int, int>, std::pair<int, int>> groups;   // (s2, q_R) or (q_L, s1) -> (first position, width) in a row
+  };
+  std::map<std::pair<int, int>, Sec> sec;  // label (n_up, n_dn) of the kept bond sector
+  void clear() { bond = 0; direction = -1; C.release(); sec.clear(); }
+};
+
 struct PsiBlk { int qL, s1, s2, qR; int dL, dR, dLp, dRp; long long off_c, off_p; int qLp = -1; /* SU(2): (N, 2S) of L' */ int NLp = 0, SLp = 0; };
 
 }  // namespace dmrg
@@ -163,6 +178,7 @@ struct dmrg_ctx {
     for (auto it = right_cache.begin(); it != right_cache.end();) it = it->first <= i ? right_cache.erase(it) : std::next(it);
   }
   dmrg::SiteOpTable site_ops;
+  dmrg::CentreFactor centre;                    // dmrg_truncate_bond -> dmrg_start_vector
   // two-site problem
   std::vector<dmrg::PsiBlk> psi;
   std::map<std::array<int, 3>, int> psi_find;   // (qL, s1, s2) -> block

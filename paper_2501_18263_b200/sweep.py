@@ -2,10 +2,10 @@
 renormalisation, move on).  U(1)xU(1) and SU(2) (total spin 0) contexts.
 
 Everything on the hot path runs in the library (`dmrg_davidson`, `dmrg_renormalize`, the environment cache).
-OUTSIDE the hot path, as north_star allows ("the truncation SVD is outside the hot path but stays on the
-device"), this driver does with torch on the device: the SVD of the optimised two-site tensor per middle-bond
-sector, the truncation to D states, and the wave-function transformation (next start vector).  The MPS
-tensors themselves are kept as host numpy blocks, because `dmrg_mps_set_site` takes host data.
+The truncation SVD, the new site tensor and the wave-function transformation (next start vector) are library calls
+too in the `native` mode (`dmrg_truncate_bond`, `dmrg_start_vector`; U(1)xU(1), default for D <= 512).  Otherwise, as
+north_star allows ("the truncation SVD is outside the hot path but stays on the device"), this driver does them with
+torch on the device and keeps the MPS tensors as host numpy blocks, because `dmrg_mps_set_site` takes host data.
 
 SU(2): the same steps on reduced (multiplet) blocks.  The middle-bond label of a block is (N, 2S') of
 L' = L + site k; the SVD factors are plain isometries on multiplets; a singular value is the total weight of
@@ -26,10 +26,17 @@ def _qadd(q, s):
 
 
 class TwoSiteSweep:
-    def __init__(self, d, T, V, mps, D, e_core=0.0):
-        """d: binding.DMRG (U(1)); mps: inputs.MPSInput positioned at bond (mps.k, mps.k+1)."""
+    def __init__(self, d, T, V, mps, D, e_core=0.0, native=None):
+        """d: binding.DMRG; mps: inputs.MPSInput / SU2MPSInput positioned at bond (mps.k, mps.k+1).
+        native: do the truncation and the wave-function transformation with the library calls dmrg_truncate_bond /
+        dmrg_start_vector (no torch.linalg, no host copy of the site tensors) instead of the torch code below.
+        Default: yes for U(1)xU(1) contexts with D <= 512, where the bond sectors fit the library's shared-memory
+        Jacobi SVD; the torch path stays for SU(2) and for large D (where the library's SVD is correct but slow)."""
         self.d, self.D = d, D
         self.su2 = bool(getattr(d, "su2", False))
+        self.native = (not self.su2 and D <= 512) if native is None else bool(native)
+        if self.native and self.su2:
+            raise ValueError("the library's truncation step is U(1)xU(1) only")
         self.L = mps.L
         self.k = mps.k
         self.sectors = [dict(s) for s in mps.sectors]
@@ -89,6 +96,20 @@ class TwoSiteSweep:
         self.last_psi = x                      # the optimised two-site wavefunction this step truncates (tests)
         if direction is None:
             self.guess = x
+            return E
+        if self.native:
+            # ---- the library's truncation step: SVD per bond sector, selection, new site tensor, all on the device ----
+            w, _ = d.truncate_bond(x, direction, self.D)
+            self.trunc.append(w)
+            self.sectors[k] = d.bond_sectors(k)
+            t0 = self._tick("SVD", t0)
+            d.renormalize(direction)
+            self.k = k + 1 if direction == 0 else k - 1
+            t0 = self._tick("Ren+Tables", t0)
+            y = d.start_vector()
+            nrm = torch.linalg.norm(y)
+            self.guess = y / nrm if float(nrm) > 0 else None
+            self._tick("StVec", t0)
             return E
         # ---- SVD per middle-bond sector q_mid = qL + q(s1) ----
         groups = {}
