@@ -117,3 +117,28 @@ def test_config2_full_size_elementwise_parity():
     ref = orc.apply(v)
     assert np.linalg.norm(got - ref) / np.linalg.norm(ref) <= 1e-11
     assert np.abs(dg - orc.diag()).max() <= 1e-10
+
+
+def test_sectors_above_one_tile_elementwise():
+    """L = 14, N = (7, 7), D = 1500: bond sectors of 250, 150, 90 and 30 states, so that outputs are cut into several
+    tiles per dimension (256 = 128 + 128, 152 = 128 + 32, 96 = 64 + 32, 32) and split along K.  The whole vector
+    against the CPU oracle, element by element and block by block (~40 s of oracle time), and the diagonal."""
+    import torch
+    from helpers import assert_blocks_close
+    from oracle import dmrg as odmrg
+    from paper_2501_18263_b200.binding import DMRG
+    L, n_el, D = 14, 7, 1500
+    T, V = inputs.make_integrals(L, 5)
+    mps = inputs.make_mps(L, n_el, n_el, D, L // 2, seed=5)
+    assert sorted(set(mps.sectors[L // 2 - 1].values()), reverse=True)[:4] == [250, 150, 90, 30]
+    pb = inputs.psi_blocks(mps)
+    v = inputs.make_psi0(mps, 1)
+    d = DMRG(L, n_el, n_el)
+    d.setup(T, V, mps)
+    got = d.heff_apply(torch.from_numpy(v).cuda()).cpu().numpy()
+    dg = d.heff_diag().cpu().numpy()
+    d.close()
+    orc = odmrg.TwoSiteOracle(T, V, n_el, n_el, mps.k, mps.sectors, mps.left, mps.right, pb)
+    orc.build_env()
+    assert_blocks_close(got, orc.apply(v), [b[4] * b[5] for b in pb], 1e-11)
+    assert np.abs(dg - orc.diag()).max() <= 1e-10
