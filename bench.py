@@ -134,13 +134,31 @@ def time_oracle_sample(d, T, V, mps, psi0, steps, warmup, nblocks=10, max_elems=
         one_pass()
     dt = (time.perf_counter() - t0) / max(steps, 1)
     flops = float(sum(bf[i] for i in idxs))
+    # the same products through the oracle's plain C + OpenMP loop (oracle/cproducts.c: two triple loops per product, no
+    # BLAS), list of products gathered before the timed region
+    c_line = None
+    try:
+        from oracle import clevel
+        pl = clevel.ProductList(terms, psi, {kk: np.zeros_like(psi[kk]) for kk in keys})
+        ref = one_pass()
+        got = pl.run()
+        err = max(float(np.abs(got[kk] - ref[kk]).max()) / max(1.0, float(np.abs(ref[kk]).max())) for kk in keys)
+        t1 = time.perf_counter()
+        for _ in range(steps):
+            pl.run()
+        dtc = (time.perf_counter() - t1) / max(steps, 1)
+        c_line = {"value": flops / dtc * 1e-9, "unit": UNIT, "cores": int(os.cpu_count()), "kind": "oracle, contraction loop in "
+                  "plain C + OpenMP (oracle/cproducts.c), same sample and flop count", "ms_per_pass": dtc * 1e3,
+                  "max_rel_dev_from_numpy_loop": err}
+    except Exception as e:      # no C compiler on the box: the numpy figure stands alone
+        c_line = {"unavailable": str(e)[:200]}
     return {"value": flops / dt * 1e-9, "unit": UNIT, "cores": _host_threads(), "kind": "oracle",
             "sample": "the bench configuration itself: %d of its %d psi' output blocks (dims %s), %.3f %% of the analytic flops of one "
                       "H_eff.psi, %.2f s of oracle time per pass; flops = the library's task-list count for those blocks "
                       "(dmrg_block_flops), operator blocks exported from the library's environments before the timed region"
                       % (len(idxs), len(pb), ", ".join("%dx%d" % (pb[i][4], pb[i][5]) for i in idxs),
                          100.0 * flops / float(bf.sum()), dt),
-            "ms_per_apply": dt * 1e3, "sample_flops": flops, "apply_flops": float(bf.sum())}
+            "ms_per_apply": dt * 1e3, "sample_flops": flops, "apply_flops": float(bf.sum()), "c_openmp": c_line}
 
 
 def _workload(cfg, mps, n_up, n_dn, su2, D):
@@ -352,7 +370,20 @@ def run_ours(args):
             s2 = d.stats()
             extra["renormalize_step"] = {"ms": s2["renorm_ms"], "gflop": s2["flops_renorm"] * 1e-9,
                                          "tflops": s2["flops_renorm"] / (s2["renorm_ms"] * 1e-3) * 1e-12,
-                                         "includes": "host planning of the step + all launches + sync"}
+                                         "includes": "host planning of the step + all launches + sync; first call: "
+                                                     "the caller's allocator has no cached block for the workspace",
+                                         "call_wall_ms": s2["last_build_ms"]}
+            # the same step in the state a sweep sees: one step back (site k+2 is still right-canonical), then again
+            d.renormalize(1)
+            d.mps_set_site(mps.k, 0, inputs.make_left_site(mps.sectors, mps.k, c["seed"]))
+            d.renormalize(0)
+            torch.cuda.synchronize()
+            s3 = d.stats()
+            extra["renormalize_step"].update({
+                "ms_steady": s3["renorm_ms"], "tflops_steady": s3["flops_renorm"] / (s3["renorm_ms"] * 1e-3) * 1e-12,
+                "call_wall_ms_steady": s3["last_build_ms"],
+                "call_wall_includes": "dmrg_renormalize as a sweep calls it: blocking step + task list, complementary "
+                                      "operators and diagonal of the next two-site problem"})
 
     # DRAM bytes per launch of the dominant kernel: written next to the committed ncu --set full summary of this
     # workload (profiles/gemm128_traffic.json, dram__bytes_read.sum + dram__bytes_write.sum); default config only.

@@ -400,6 +400,7 @@ void Planner::finish(Plan* plan, cudaStream_t st) {
   plan->ws_half = ws_max_;
   if (ws_max_ > 0) plan->workspace.allocate(al_, (size_t)ws_max_ * (two_halves ? 2 : 1));
   double* ws = plan->workspace.p;
+  pt.lap("workspace allocation (the caller's allocator)");
   if (std::getenv("DMRG_B200_PLAN_STATS")) plan->print_stats = true;
 
   // ---- split-K: heavy outputs are cut into parts along their (segment, repeat) list so that one launch
@@ -414,36 +415,49 @@ void Planner::finish(Plan* plan, cudaStream_t st) {
     // about as long per k-chunk as a 64x128 one.  Outputs are cut so that no tile part exceeds 1/16 of
     // the per-SM share of the chunk.
     double total = 0;
-    std::vector<double> ks(hv.size()), mxa(hv.size());
-    for (size_t i = 0; i < hv.size(); ++i) {
+    std::vector<double> ks(hv.size()), mxa(hv.size()), contrib(hv.size());
+    const long long nhv = (long long)hv.size();
+    // (per-output terms in parallel, summed in index order below: the plan does not depend on the thread count)
+#pragma omp parallel for schedule(static) if (nhv > 4096)
+    for (long long i = 0; i < nhv; ++i) {
       double k = 0;
       for (auto& hs : hv[i].segs) k += (double)hs.s.K * hs.s.count;
       ks[i] = k;
-      std::vector<std::pair<int, int>> rs, cs;
+      static thread_local std::vector<std::pair<int, int>> rs, cs;
+      rs.clear(); cs.clear();
       split_dim(hv[i].o.M, rs); split_dim(hv[i].o.N, cs);
-      double mx = 0;
+      double mx = 0, sum = 0;
       for (auto& r : rs) for (auto& c : cs) {
         double t = std::max(8192.0, (double)GEMM_DIMS[r.second] * GEMM_DIMS[c.second]);
-        total += k * t * hv[i].batch;
+        sum += k * t * hv[i].batch;
         mx = std::max(mx, t);
       }
       mxa[i] = mx;
+      contrib[i] = sum;
     }
+    for (long long i = 0; i < nhv; ++i) total += contrib[i];
     const double wstar = total / (148.0 * 32.0);
-    std::vector<HOut> ex;
-    long long sc_used = 0;
-    for (size_t i = 0; i < hv.size(); ++i) {
-      HOut& h = hv[i];
+    // the parts of every heavy output are built on host threads (scratch offsets relative to the output's own
+    // partial tiles), then appended in output order with the running scratch offset
+    struct Split { long long out; int ns; std::vector<HOut> parts; HRed rd; long long sc_need = 0; };
+    std::vector<Split> sp;                      // the outputs that are cut, in output order
+    for (long long i = 0; i < nhv; ++i) {
       long long units = 0;
-      for (auto& hs : h.segs) units += hs.s.count;
+      for (auto& hs : hv[i].segs) units += hs.s.count;
       int ns = wstar > 0 ? (int)std::ceil(ks[i] * mxa[i] / wstar) : 1;
       ns = (int)std::min<long long>(std::min(ns, 32), units);
-      if (ns <= 1) { ex.push_back(std::move(h)); continue; }
+      if (ns > 1) { sp.emplace_back(); sp.back().out = i; sp.back().ns = ns; }
+    }
+    const long long nsp = (long long)sp.size();
+#pragma omp parallel for schedule(dynamic, 64) if (nsp > 1024)
+    for (long long q = 0; q < nsp; ++q) {
+      Split& S = sp[q];
+      const long long i = S.out;
+      const int ns = S.ns;
+      HOut& h = hv[i];
       const long long mn = (long long)h.o.M * h.o.N;
-      HRed rd{};
-      rd.d.C = h.o.C; rd.d.bsC = h.o.bsC; rd.d.M = h.o.M; rd.d.N = h.o.N; rd.d.ldc = h.o.ldc;
-      rd.d.nparts = ns - 1; rd.d.batch = h.batch; rd.p_off = sc_used;
-      reds[ci].push_back(rd);
+      S.rd.d.C = h.o.C; S.rd.d.bsC = h.o.bsC; S.rd.d.M = h.o.M; S.rd.d.N = h.o.N; S.rd.d.ldc = h.o.ldc;
+      S.rd.d.nparts = ns - 1; S.rd.d.batch = h.batch; S.rd.p_off = 0;
       const double target = ks[i] / ns;
       size_t si = 0; int rep = 0;      // cursor into the (segment, repeat) list
       for (int p = 0; p < ns; ++p) {
@@ -451,7 +465,7 @@ void Planner::finish(Plan* plan, cudaStream_t st) {
         part.o = h.o; part.c_ws = false; part.batch = h.batch; part.work = 0;
         if (p > 0) {
           part.c_sc = true;
-          part.o.C = reinterpret_cast<double*>(sc_used + (long long)(p - 1) * h.batch * mn);
+          part.o.C = reinterpret_cast<double*>((long long)(p - 1) * h.batch * mn);
           part.o.bsC = mn; part.o.ldc = h.o.N; part.o.accumulate = 0;
         }
         double got = 0;
@@ -476,10 +490,25 @@ void Planner::finish(Plan* plan, cudaStream_t st) {
           rep += take;
           if (rep >= hs.s.count) { rep = 0; ++si; }
         }
-        if (!part.segs.empty() || p == 0) ex.push_back(std::move(part));
-        else reds[ci].back().d.nparts = std::min(reds[ci].back().d.nparts, p - 1);
+        if (!part.segs.empty() || p == 0) S.parts.push_back(std::move(part));
+        else S.rd.d.nparts = std::min(S.rd.d.nparts, p - 1);
       }
-      sc_used += (long long)(ns - 1) * h.batch * mn;
+      S.sc_need = (long long)(ns - 1) * h.batch * mn;
+    }
+    std::vector<HOut> ex;
+    ex.reserve(hv.size());
+    long long sc_used = 0;
+    size_t nq = 0;
+    for (size_t i = 0; i < hv.size(); ++i) {
+      if (nq >= sp.size() || sp[nq].out != (long long)i) { ex.push_back(std::move(hv[i])); continue; }
+      Split& S = sp[nq++];
+      S.rd.p_off = sc_used;
+      reds[ci].push_back(S.rd);
+      for (auto& part : S.parts) {
+        if (part.c_sc) part.o.C = reinterpret_cast<double*>(reinterpret_cast<long long>(part.o.C) + sc_used);
+        ex.push_back(std::move(part));
+      }
+      sc_used += S.sc_need;
     }
     hv.swap(ex);
     scratch_max = std::max(scratch_max, sc_used);
@@ -601,12 +630,19 @@ void Planner::finish(Plan* plan, cudaStream_t st) {
   }
   fused_.clear();
   fused_index_.clear();
-  auto build = [&](std::vector<HOut>& hv, Phase& ph, double* ws) {
-    std::vector<GOut> outs;
-    std::vector<GSeg> segs;
+  // host side of one phase of one chunk: descriptors and per-shape tile lists (heaviest first).  Independent of every
+  // other (chunk, phase), so all of them are built on host threads at once; the uploads follow in order.
+  struct Built { std::vector<GOut> outs; std::vector<GSeg> segs; std::vector<GTile> tiles[GEMM_NSHAPES]; };
+  auto build_host = [&](std::vector<HOut>& hv, Phase& ph, double* ws, Built& bt) {
+    std::vector<GOut>& outs = bt.outs;
+    std::vector<GSeg>& segs = bt.segs;
     struct TW { GTile t; double w; };
     std::vector<TW> tw[GEMM_NSHAPES];
     outs.reserve(hv.size());
+    size_t nseg = 0;
+    for (auto& h : hv) nseg += h.segs.size();
+    segs.reserve(nseg);
+    std::vector<std::pair<int, int>> rs, cs;
     for (size_t oi = 0; oi < hv.size(); ++oi) {
       HOut& h = hv[oi];
       GOut o = h.o;
@@ -624,7 +660,7 @@ void Planner::finish(Plan* plan, cudaStream_t st) {
       o.seg_end = (int)segs.size();
       outs.push_back(o);
       if (o.seg_begin == o.seg_end) continue;   // nothing to add: the kernel needs >= 1 k-chunk per tile
-      std::vector<std::pair<int, int>> rs, cs;
+      rs.clear(); cs.clear();
       split_dim(o.M, rs);
       split_dim(o.N, cs);
       for (int b = 0; b < h.batch; ++b)
@@ -640,21 +676,34 @@ void Planner::finish(Plan* plan, cudaStream_t st) {
     }
     for (int s = 0; s < GEMM_NSHAPES; ++s) {
       std::stable_sort(tw[s].begin(), tw[s].end(), [](const TW& a, const TW& b) { return a.w > b.w; });
-      std::vector<GTile> tiles(tw[s].size());
-      for (size_t i = 0; i < tw[s].size(); ++i) tiles[i] = tw[s][i].t;
-      ph.ntiles[s] = (int)tiles.size();
-      if (!tiles.empty()) ph.tiles[s].upload(al_, tiles, st);
+      bt.tiles[s].resize(tw[s].size());
+      for (size_t i = 0; i < tw[s].size(); ++i) bt.tiles[s][i] = tw[s][i].t;
+      ph.ntiles[s] = (int)bt.tiles[s].size();
     }
-    ph.outs.upload(al_, outs, st);
-    ph.segs.upload(al_, segs, st);
+  };
+  auto upload_built = [&](Built& bt, Phase& ph) {
+    for (int s = 0; s < GEMM_NSHAPES; ++s)
+      if (!bt.tiles[s].empty()) ph.tiles[s].upload(al_, bt.tiles[s], st);
+    ph.outs.upload(al_, bt.outs, st);
+    ph.segs.upload(al_, bt.segs, st);
+    bt = Built{};
   };
   pt.lap("fused upload");
   plan->chunks.resize(chunks_.size());
   struct PS { double act = 0, full = 0; long long tiles = 0; } ps[2][GEMM_NSHAPES];
-  for (size_t c = 0; c < chunks_.size(); ++c) {
+  std::vector<Built> built(2 * chunks_.size());
+  const long long nbuild = (long long)built.size();
+#pragma omp parallel for schedule(dynamic, 1) if (nbuild > 2)
+  for (long long i = 0; i < nbuild; ++i) {
+    const size_t c = (size_t)i / 2;
     double* wsc = ws + ((c & 1) ? ws_max_ : 0);   // chunk c works in workspace half c & 1
-    build(chunks_[c].p1, plan->chunks[c].p1, wsc);
-    build(chunks_[c].p2, plan->chunks[c].p2, wsc);
+    if (i & 1) build_host(chunks_[c].p2, plan->chunks[c].p2, wsc, built[i]);
+    else build_host(chunks_[c].p1, plan->chunks[c].p1, wsc, built[i]);
+  }
+  pt.lap("chunk tile lists (host threads)");
+  for (size_t c = 0; c < chunks_.size(); ++c) {
+    upload_built(built[2 * c], plan->chunks[c].p1);
+    upload_built(built[2 * c + 1], plan->chunks[c].p2);
     if (!reds[c].empty()) {
       std::vector<RedDesc> rd;
       int mb = 1;
@@ -683,7 +732,7 @@ void Planner::finish(Plan* plan, cudaStream_t st) {
           fprintf(stderr, "plan phase %d shape %dx%d tiles %lld flops %.4g full-tile flops %.4g (fill %.3f)\n", p + 1,
                   GEMM_DIMS[sh / 3], GEMM_DIMS[sh % 3], ps[p][sh].tiles, ps[p][sh].act, ps[p][sh].full,
                   ps[p][sh].act / ps[p][sh].full);
-  pt.lap("chunk tile lists + upload");
+  pt.lap("chunk uploads");
   chunks_.clear();
   pt.lap("free host items");
 }
