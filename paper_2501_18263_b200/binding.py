@@ -145,7 +145,10 @@ class DMRG:
         # do not.  Left alone when the user has configured the allocator.
         if "PYTORCH_CUDA_ALLOC_CONF" not in os.environ and "PYTORCH_ALLOC_CONF" not in os.environ:
             try:
-                torch.cuda.memory._set_allocator_settings("expandable_segments:True")
+                setter = getattr(torch._C, "_accelerator_setAllocatorSettings", None)      # torch >= 2.9
+                if setter is None:
+                    setter = torch.cuda.memory._set_allocator_settings
+                setter("expandable_segments:True")
             except Exception:      # an older torch: keep its default
                 pass
 

@@ -296,9 +296,14 @@ static uint64_t workspace_cap(const dmrg_ctx* ctx) {
   if (ctx->cfg.workspace_bytes) return ctx->cfg.workspace_bytes;
   size_t fr = 0, tot = 0;
   if (cudaMemGetInfo(&fr, &tot) != cudaSuccess) return 16ull << 30;
-  const uint64_t mine = ctx->al.live_bytes;
+  // the context's workspace arena is what the cap is about: it does not count as memory taken (while no plan holds it)
+  const uint64_t arena = ctx->ws_arena.in_use ? 0 : 8ull * ctx->ws_arena.buf.n;
+  const uint64_t mine = ctx->al.live_bytes > arena ? ctx->al.live_bytes - arena : 0;
   const uint64_t rest = tot > mine ? tot - mine : 0;
-  return std::min<uint64_t>(std::max<uint64_t>(rest / 5 * 2, 1ull << 30), 64ull << 30);
+  const uint64_t cap = std::min<uint64_t>(std::max<uint64_t>(rest / 5 * 2, 1ull << 30), 64ull << 30);
+  // an arena of 60-100 % of that is kept as it is: plans are then cut to fit it and it is never reallocated in a sweep
+  if (arena >= cap / 5 * 3 && arena <= cap) return arena;
+  return cap;
 }
 
 static inline uint64_t pack_key(int a, int b, int c, int d, int e, int f) {
@@ -465,7 +470,7 @@ std::unique_ptr<BlockSide> renormalize_block(dmrg_ctx* ctx, const BlockSide& old
   pt.lap("group + pre-sum");
   // ---- emit the triple products  new(q2' <- q1') += alpha * W2^T op(S)(q2 <- q1) W1 ----
   const uint64_t cap = workspace_cap(ctx);
-  Planner planner(&ctx->al, cap);
+  Planner planner(&ctx->al, cap, &ctx->ws_arena);
   for (auto& f : fgs) {
     OpClass& D = *B.cls[f.g.dk];
     const OpClass& S = *f.src;
@@ -949,7 +954,7 @@ void prepare_superblock(dmrg_ctx* ctx, cudaStream_t st) {
 
   // ---- tasks of PAPER.md Eq. (8): (term group x psi block) -> contraction items + diagonal tasks ----
   const uint64_t cap = workspace_cap(ctx);
-  Planner planner(&ctx->al, cap);
+  Planner planner(&ctx->al, cap, &ctx->ws_arena);
   std::vector<std::vector<DiagTask>> dtasks(ctx->psi.size());
   int64_t n_tasks = 0, n_groups = 0;
   // psi blocks outermost: the items that apply the same operator run to the same psi block (different term

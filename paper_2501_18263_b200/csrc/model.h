@@ -187,6 +187,7 @@ struct dmrg_ctx {
   long long psi_n = 0, psi_np = 0;
   dmrg::DevArray<dmrg::PsiBlockDev> d_psi_blocks;
   dmrg::DevArray<double> psi_in_p, psi_out_p, diag_p;
+  dmrg::WsArena ws_arena;                       // declared before every plan that may lease it (destroyed after them)
   dmrg::Plan apply_plan;
   // output-block sharding of the apply over ranks (dmrg_set_shard); psi_owner[block] = rank that computes it
   int shard_rank = 0, shard_count = 1;

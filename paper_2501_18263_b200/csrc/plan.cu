@@ -398,8 +398,25 @@ void Planner::finish(Plan* plan, cudaStream_t st) {
   plan->n_products = n_products_;
   const bool two_halves = chunks_.size() > 1;
   plan->ws_half = ws_max_;
-  if (ws_max_ > 0) plan->workspace.allocate(al_, (size_t)ws_max_ * (two_halves ? 2 : 1));
-  double* ws = plan->workspace.p;
+  double* ws = nullptr;
+  if (ws_max_ > 0) {
+    const size_t need = (size_t)ws_max_ * (two_halves ? 2 : 1);
+    if (arena_ && !arena_->in_use) {
+      // grow when the plan needs more; give the block back when it is far larger than what this plan may use at all
+      // (the cap follows the memory the context has left: environment blocks may have grown since)
+      const size_t limit = std::max<size_t>(need, 2 * (size_t)cap_);
+      if (arena_->buf.n < need || arena_->buf.n > limit + limit / 4) {
+        arena_->buf.release();
+        arena_->buf.allocate(al_, need);
+      }
+      arena_->in_use = true;
+      plan->lease.reset(arena_);
+      ws = arena_->buf.p;
+    } else {
+      plan->workspace.allocate(al_, need);
+      ws = plan->workspace.p;
+    }
+  }
   pt.lap("workspace allocation (the caller's allocator)");
   if (std::getenv("DMRG_B200_PLAN_STATS")) plan->print_stats = true;
 

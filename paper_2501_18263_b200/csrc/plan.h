@@ -10,6 +10,7 @@
 #pragma once
 #include <cstdlib>
 #include <map>
+#include <memory>
 #include <tuple>
 
 #include "common.h"
@@ -95,13 +96,25 @@ struct Exec {
   ~Exec();
 };
 
+// Workspace arena of a context: the intermediates of one plan at a time live in ONE device block that outlasts the
+// plans (a blocking step, then the two-site problem of the next bond, ...), instead of one allocation of tens of GB
+// per plan through the caller's allocator (measured: 90 ms of cudaMalloc per fresh workspace behind torch, and
+// fragmentation over a sweep).  A plan leases it; a second plan built while the lease is out allocates its own.
+struct WsArena {
+  DevArray<double> buf;
+  bool in_use = false;
+};
+struct WsArenaRelease { void operator()(WsArena* a) const { if (a) a->in_use = false; } };
+using WsLease = std::unique_ptr<WsArena, WsArenaRelease>;
+
 // One kernel launch of a plan, timed with CUDA events (dmrg_apply_profile).
 struct LaunchRecord { int chunk, phase, shape, ntiles; double flops; float ms; };
 
 struct Plan {
   std::vector<Chunk> chunks;
   FusedPhase fused;
-  DevArray<double> workspace, scratch;
+  DevArray<double> workspace, scratch;   // workspace: only when the plan could not lease the context's arena
+  WsLease lease;                         // the arena this plan's intermediates live in (released with the plan)
   bool print_stats = false;   // DMRG_B200_PLAN_STATS: per-shape tile fill printed when a plan is built
   long long ws_half = 0;   // elements per workspace half (two halves when there are several chunks)
   double flops_analytic = 0, flops_executed = 0, bytes_intermediate = 0;
@@ -116,13 +129,14 @@ struct Plan {
   void run(cudaStream_t st, int64_t* launch_counter, Exec* ex = nullptr) const;
   // Same launches, each bracketed by events (shape -1 = split-K reduction).  Synchronises `st`.
   void run_profiled(cudaStream_t st, std::vector<LaunchRecord>* out) const;
-  void clear() { chunks.clear(); fused.clear(); workspace.release(); scratch.release(); }
+  void clear() { chunks.clear(); fused.clear(); workspace.release(); scratch.release(); lease.reset(); }
 };
 
 class Planner {
  public:
   // A chunk may use half the cap: consecutive chunks alternate between two workspace halves.
-  Planner(Allocator* al, uint64_t workspace_cap_bytes) : al_(al), cap_(workspace_cap_bytes / 16) {}
+  Planner(Allocator* al, uint64_t workspace_cap_bytes, WsArena* arena = nullptr)
+      : al_(al), cap_(workspace_cap_bytes / 16), arena_(arena) {}
   void add(const Item& it);
   // Uploads descriptors, allocates the workspace and patches workspace-relative pointers.
   void finish(Plan* plan, cudaStream_t st);
@@ -175,6 +189,7 @@ class Planner {
   HOut& p2_out(HChunk& ch, const Item& it, int b0, int cnt, int M, int N);
   Allocator* al_;
   long long cap_;
+  WsArena* arena_ = nullptr;
   std::vector<HChunk> chunks_;
   long long ws_max_ = 0;
   double fa_ = 0, fe_ = 0, bi_ = 0, fshared_ = 0;
