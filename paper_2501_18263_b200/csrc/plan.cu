@@ -429,8 +429,8 @@ void Planner::finish(Plan* plan, cudaStream_t st) {
   for (size_t ci = 0; ci < chunks_.size(); ++ci) {
     std::vector<HOut>& hv = chunks_[ci].p2;
     // cost model of one tile: k-chunks x max(tile area, 8192) -- a narrow tile is latency-bound and takes
-    // about as long per k-chunk as a 64x128 one.  Outputs are cut so that no tile part exceeds 1/16 of
-    // the per-SM share of the chunk.
+    // about as long per k-chunk as a 64x128 one.  Outputs are cut so that no tile part exceeds 1/64 of
+    // the per-SM share of the chunk (at most 32 parts per output).
     double total = 0;
     std::vector<double> ks(hv.size()), mxa(hv.size()), contrib(hv.size());
     const long long nhv = (long long)hv.size();
@@ -453,7 +453,9 @@ void Planner::finish(Plan* plan, cudaStream_t st) {
       contrib[i] = sum;
     }
     for (long long i = 0; i < nhv; ++i) total += contrib[i];
-    const double wstar = total / (148.0 * 32.0);
+    // (measured at 1/8, 1/16, 1/32, 1/64, 1/96, 1/128 of the per-SM share: configs[3] 527.9 / 496.8 / 488.4-489.3 /
+    // 486.2-487.2 / 488.6 / 491.0 ms; configs[2] and SU(2) configs[3] are 1 % faster at 1/64 than at 1/32 as well)
+    const double wstar = total / (148.0 * 64.0);
     // the parts of every heavy output are built on host threads (scratch offsets relative to the output's own
     // partial tiles), then appended in output order with the running scratch offset
     struct Split { long long out; int ns; std::vector<HOut> parts; HRed rd; long long sc_need = 0; };
