@@ -557,9 +557,10 @@ void Planner::finish(Plan* plan, cudaStream_t st) {
     }
     for (size_t i = 0; i < fused_.size(); ++i) {
       HFOut& o = fused_[i];
-      // aim at ~3 work items per resident warp of the class, all of about the same length
+      // aim at ~6 work items per resident warp of the class, all of about the same length (measured at 1.5 / 3 / 6 /
+      // 12 / 24: configs[1] 0.598 / 0.543 / 0.532 / 0.531 / 0.533 ms, configs[2] 13.49 / 13.33 / 13.25 / 13.25 / 13.25 ms)
       const int rows = FUSED_STRIP;
-      const double target = std::max(cls_total[cls[i]] / (148.0 * fused_warps_per_sm(cls[i]) * 3.0), 1.0);
+      const double target = std::max(cls_total[cls[i]] / (148.0 * fused_warps_per_sm(cls[i]) * 6.0), 1.0);
       long long units = 0;
       for (auto& t : o.tasks) units += t.count;
       int ns = (int)std::min<long long>(std::min<long long>((long long)std::ceil(cost[i] / target), 64), units);
